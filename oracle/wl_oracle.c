@@ -1,0 +1,280 @@
+/*
+ * wl_oracle.c -- FP64 CPU oracle for the worldline-numerics hot path.
+ *
+ * TEST INFRASTRUCTURE, NOT PRODUCT.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may build, load or call this
+ * file.  It shares no code with paper_1407_7486_b200/csrc (the CUDA path) and
+ * never receives a value computed by it.
+ *
+ * What it is: the definition of the estimator, written out in the order and
+ * notation of the paper (arXiv:1407.7486, /root/reference/PAPER.md), in double
+ * precision, with no blocking, fusion or reordering:
+ *
+ *   x_i   = x_cm + sqrt(T) y_i                          eq. (8),
+ *   phase = sum_i  g(|m_i|) (m_i x d_i)                  eq. (21)-(24)
+ *           m_i = (x_i + x_{i+1})/2,  d_i = x_{i+1} - x_i, i+1 taken mod N,
+ *           g(rho) = e A_phi(rho)/rho = e Phi(rho)/(2 pi rho^2)   (one-point
+ *           midpoint rule for the t-integral of eq. (24); reading A2)
+ *   spin  = (T/N) sum_i e B(|x_i|)                       eq. (31)-(33)
+ *   W     = cos(phase) cosh(spin)                        eq. (18)
+ *   S_g   = sum of W over loops [g N_l/G, (g+1) N_l/G)   eq. (60)
+ *   <W>   = (sum_g S_g)/N_l                              eq. (61)-(62)
+ *   err   = sqrt(sum_g (<W>_g - <W>)^2 / (G (G-1)))      eq. (63)
+ *
+ * plus the unit-loop generator (d-loops, steps (1)-(5), eq. (10)-(11),
+ * PAPER.md:65-81) driven by Philox4x32-10 (reading A11).
+ *
+ * Pins (tests/test_oracle_*.py, all -m "not gpu"): zero field, uniform-field
+ * shoelace area, finite-N uniform closed form, Stokes flux of the sech^2
+ * profile by independent quadrature, mpmath evaluation of the profile,
+ * lambda->infinity limit, rotation/relabelling invariances, 4-point brute
+ * force, sampler moments and a Fourier-mode twin, Philox known answers.
+ * No function here is "parity unpinned".
+ *
+ * OpenMP is used only to run independent loops on several cores; every sum is
+ * taken serially in index order.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define WLO_PROFILE_UNIFORM 0
+#define WLO_PROFILE_SECH2 1
+
+/* ------------------------------------------------------------------------- */
+/* Field profiles.  e is folded into the field strength: only eB, eB0 enter.  */
+/* ------------------------------------------------------------------------- */
+
+/* h(u) = [u tanh u - ln cosh u]/u^2, so that for B = B0 sech^2(rho/lambda),
+ * Phi(rho) = 2 pi B0 [lambda rho tanh(rho/lambda) - lambda^2 ln cosh(rho/lambda)]
+ * (BASELINE.json config 1) gives g = e Phi/(2 pi rho^2) = eB0 h(rho/lambda).
+ * u < 0.1: Maclaurin series (next term 3.3e-3 u^12 < 4e-15);
+ * else the cancellation-free form with E = exp(-2u) (never calls cosh).      */
+static double sech2_h(double u)
+{
+    if (u < 0.1) {
+        double w = u * u;
+        return 0.5 + w * (-1.0 / 4.0 + w * (1.0 / 9.0 + w * (-17.0 / 360.0
+                 + w * (31.0 / 1575.0 + w * (-691.0 / 85050.0)))));
+    }
+    double E = exp(-2.0 * u);
+    double P = M_LN2 - log1p(E) - 2.0 * u * E / (1.0 + E);
+    return P / (u * u);
+}
+
+/* sech^2(u) = 4E/(1+E)^2, E = exp(-2u). */
+static double sech2_b(double u)
+{
+    double E = exp(-2.0 * u);
+    return 4.0 * E / ((1.0 + E) * (1.0 + E));
+}
+
+/* g(rho) = e A_phi(rho)/rho   (eq. (14), (23)) */
+double wlo_field_g(int profile, const double *params, double rho)
+{
+    if (profile == WLO_PROFILE_UNIFORM)
+        return 0.5 * params[0];                 /* A = (B/2)(-y, x) */
+    return params[0] * sech2_h(rho / params[1]);
+}
+
+/* b(rho) = e B_z(rho)         (eq. (13), (15)) */
+double wlo_field_b(int profile, const double *params, double rho)
+{
+    if (profile == WLO_PROFILE_UNIFORM)
+        return params[0];
+    return params[0] * sech2_b(rho / params[1]);
+}
+
+/* ------------------------------------------------------------------------- */
+/* One Wilson loop at one (T, x_cm).  y: [N][2] unit loop.                    */
+/* ------------------------------------------------------------------------- */
+void wlo_loop_phase_spin(int profile, const double *params,
+                         const double *y, int N, double T, double cx, double cy,
+                         double *phase_out, double *spin_out)
+{
+    double s = sqrt(T);
+    double phase = 0.0, spin = 0.0;
+    for (int i = 0; i < N; ++i) {
+        int j = (i + 1) % N;
+        double xi_x = cx + s * y[2 * i], xi_y = cy + s * y[2 * i + 1];
+        double xj_x = cx + s * y[2 * j], xj_y = cy + s * y[2 * j + 1];
+        double m_x = 0.5 * (xi_x + xj_x), m_y = 0.5 * (xi_y + xj_y);
+        double d_x = xj_x - xi_x, d_y = xj_y - xi_y;
+        phase += wlo_field_g(profile, params, sqrt(m_x * m_x + m_y * m_y)) * (m_x * d_y - m_y * d_x);
+        spin += wlo_field_b(profile, params, sqrt(xi_x * xi_x + xi_y * xi_y));
+    }
+    *phase_out = phase;
+    *spin_out = T / (double)N * spin;
+}
+
+/* ------------------------------------------------------------------------- */
+/* Whole ensemble on a (T, rho_cm[, phi_cm]) grid.                            */
+/*   loops      [n_loops][N][2]                                               */
+/*   W_mean     [n_T][n_rho]                                                  */
+/*   group_sums [G][n_T][n_rho]                                               */
+/*   W_loop, phase_loop, spin_loop: nullable, [n_loops][n_T][n_rho]           */
+/* Returns 0, or -1 on a bad argument.                                        */
+/* ------------------------------------------------------------------------- */
+int wlo_eval(int profile, const double *params,
+             const double *loops, int64_t n_loops, int N,
+             const double *T, int n_T,
+             const double *rho_cm, const double *phi_cm, int n_rho,
+             int n_groups,
+             double *W_mean, double *group_sums,
+             double *W_loop, double *phase_loop, double *spin_loop)
+{
+    if (n_loops <= 0 || N < 1 || n_T < 1 || n_rho < 1 || n_groups < 1) return -1;
+    if (n_loops % n_groups != 0) return -1;         /* equal groups */
+    const int64_t n_grid = (int64_t)n_T * n_rho;
+    const int64_t per_group = n_loops / n_groups;
+
+    double *W = W_loop ? W_loop : (double *)malloc(sizeof(double) * n_loops * n_grid);
+    if (!W) return -1;
+
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t l = 0; l < n_loops; ++l) {
+        const double *y = loops + l * (int64_t)N * 2;
+        for (int t = 0; t < n_T; ++t)
+            for (int r = 0; r < n_rho; ++r) {
+                double ph = phi_cm ? phi_cm[r] : 0.0;
+                double cx = rho_cm[r] * cos(ph), cy = rho_cm[r] * sin(ph);
+                double phase, spin;
+                wlo_loop_phase_spin(profile, params, y, N, T[t], cx, cy, &phase, &spin);
+                int64_t o = l * n_grid + (int64_t)t * n_rho + r;
+                W[o] = cos(phase) * cosh(spin);
+                if (phase_loop) phase_loop[o] = phase;
+                if (spin_loop) spin_loop[o] = spin;
+            }
+    }
+
+    for (int64_t k = 0; k < n_grid; ++k) {
+        double total = 0.0;
+        for (int g = 0; g < n_groups; ++g) {
+            double S = 0.0;
+            for (int64_t l = g * per_group; l < (g + 1) * per_group; ++l) S += W[l * n_grid + k];
+            group_sums[(int64_t)g * n_grid + k] = S;
+            total += S;
+        }
+        W_mean[k] = total / (double)n_loops;
+    }
+    if (!W_loop) free(W);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------- */
+/* Jackknife finalise, eq. (60)-(63); delete-one-group means (reading A7).    */
+/*   mean, err [n_grid]; delete_one nullable [G][n_grid]                      */
+/* ------------------------------------------------------------------------- */
+int wlo_finalize(const double *group_sums, int n_groups, int64_t n_loops, int64_t n_grid,
+                 double *mean, double *err, double *delete_one)
+{
+    if (n_groups < 2 || n_loops % n_groups != 0) return -1;
+    const double G = (double)n_groups;
+    const double per_group = (double)(n_loops / n_groups);
+    for (int64_t k = 0; k < n_grid; ++k) {
+        double total = 0.0;
+        for (int g = 0; g < n_groups; ++g) total += group_sums[(int64_t)g * n_grid + k];
+        double m = total / (double)n_loops;
+        double ss = 0.0;
+        for (int g = 0; g < n_groups; ++g) {
+            double mg = group_sums[(int64_t)g * n_grid + k] / per_group;   /* eq. (60) */
+            ss += (mg - m) * (mg - m);
+            if (delete_one)
+                delete_one[(int64_t)g * n_grid + k] =
+                    (total - group_sums[(int64_t)g * n_grid + k]) / ((double)n_loops - per_group);
+        }
+        mean[k] = m;
+        err[k] = sqrt(ss / (G * (G - 1.0)));                               /* eq. (63) */
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------- */
+/* Philox4x32-10 (Salmon et al., SC'11), restated from the published          */
+/* algorithm: 10 rounds of two 32x32->64 multiplies, key bumped by the Weyl   */
+/* constants between rounds.                                                  */
+/* ------------------------------------------------------------------------- */
+void wlo_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+    uint32_t k0 = key[0], k1 = key[1];
+    for (int round = 0; round < 10; ++round) {
+        uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        uint32_t n1 = (uint32_t)p1;
+        uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        uint32_t n3 = (uint32_t)p0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* Two standard normals for (seed, loop, point): counter = (point, loop_lo,
+ * loop_hi, 0), key = (seed_lo, seed_hi); words (0,1) and (2,3) give two
+ * 53-bit uniforms in (0,1]; Box-Muller in FP64.  (reading A11.)   */
+void wlo_normal_pair(uint64_t seed, uint64_t loop, uint32_t point, double *nx, double *ny)
+{
+    uint32_t ctr[4] = { point, (uint32_t)loop, (uint32_t)(loop >> 32), 0u };
+    uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+    uint32_t w[4];
+    wlo_philox4x32_10(ctr, key, w);
+    uint64_t a = ((uint64_t)w[1] << 32) | w[0];
+    uint64_t b = ((uint64_t)w[3] << 32) | w[2];
+    double u1 = (double)((a >> 11) + 1) * 0x1.0p-53;
+    double u2 = (double)((b >> 11) + 1) * 0x1.0p-53;
+    double r = sqrt(-2.0 * log(u1));
+    double th = 6.283185307179586476925286766559 * u2;
+    *nx = r * cos(th);
+    *ny = r * sin(th);
+}
+
+/* d-loop generator.  Step (1): y_N = 0 (stored at index 0).
+ * Step (2)-(3): level k = 1..log2 N adds the odd multiples of h = N/2^k,
+ *   y_p = (y_{p-h} + y_{p+h})/2 + sigma_k n_p,  sigma_k^2 = 1/N_k = 2^-k per
+ *   component (eq. (10): exp(-(y-y_N)^2) at k = 1; eq. (11) at k > 1).
+ * Step (5): subtract the centre of mass.
+ * Writes loops [loop_begin, loop_begin + n_loops) into out[n_loops][N][2].
+ * N must be a power of two >= 2.  Returns 0 or -1.                           */
+int wlo_generate_loops(uint64_t seed, int64_t loop_begin, int64_t n_loops, int N, double *out)
+{
+    if (N < 2 || (N & (N - 1)) != 0 || n_loops < 0) return -1;
+    int log2N = 0;
+    while ((1 << log2N) < N) ++log2N;
+#pragma omp parallel for schedule(static)
+    for (int64_t q = 0; q < n_loops; ++q) {
+        double *y = out + q * (int64_t)N * 2;
+        uint64_t loop = (uint64_t)(loop_begin + q);
+        y[0] = 0.0; y[1] = 0.0;
+        for (int k = 1; k <= log2N; ++k) {
+            int h = N >> k;
+            double sigma = ldexp((k & 1) ? M_SQRT1_2 : 1.0, -(k / 2));
+            for (int p = h; p < N; p += 2 * h) {
+                int lo = p - h, hi = (p + h) % N;
+                double nx, ny;
+                wlo_normal_pair(seed, loop, (uint32_t)p, &nx, &ny);
+                y[2 * p] = 0.5 * (y[2 * lo] + y[2 * hi]) + sigma * nx;
+                y[2 * p + 1] = 0.5 * (y[2 * lo + 1] + y[2 * hi + 1]) + sigma * ny;
+            }
+        }
+        double mx = 0.0, my = 0.0;
+        for (int i = 0; i < N; ++i) { mx += y[2 * i]; my += y[2 * i + 1]; }
+        mx /= (double)N; my /= (double)N;
+        for (int i = 0; i < N; ++i) { y[2 * i] -= mx; y[2 * i + 1] -= my; }
+    }
+    return 0;
+}
+
+int wlo_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

@@ -1,0 +1,157 @@
+"""ctypes binding of oracle/wl_oracle.c (FP64 CPU oracle).
+
+TEST INFRASTRUCTURE, NOT PRODUCT: only tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference legs import this module.  It does not
+import the product package and the product package does not import it.
+
+Argument marshalling only; all arithmetic is in wl_oracle.c (each function there
+cites the PAPER.md passage it follows).
+"""
+import ctypes as C
+
+import numpy as np
+
+from . import build as _build
+
+UNIFORM = 0
+SECH2 = 1
+
+_lib = None
+_dp = C.POINTER(C.c_double)
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(_build.build())
+        L.wlo_field_g.restype = C.c_double
+        L.wlo_field_g.argtypes = [C.c_int, _dp, C.c_double]
+        L.wlo_field_b.restype = C.c_double
+        L.wlo_field_b.argtypes = [C.c_int, _dp, C.c_double]
+        L.wlo_loop_phase_spin.restype = None
+        L.wlo_loop_phase_spin.argtypes = [C.c_int, _dp, _dp, C.c_int, C.c_double, C.c_double,
+                                          C.c_double, _dp, _dp]
+        L.wlo_eval.restype = C.c_int
+        L.wlo_eval.argtypes = [C.c_int, _dp, _dp, C.c_int64, C.c_int, _dp, C.c_int, _dp, _dp,
+                               C.c_int, C.c_int, _dp, _dp, _dp, _dp, _dp]
+        L.wlo_finalize.restype = C.c_int
+        L.wlo_finalize.argtypes = [_dp, C.c_int, C.c_int64, C.c_int64, _dp, _dp, _dp]
+        L.wlo_philox4x32_10.restype = None
+        L.wlo_philox4x32_10.argtypes = [C.POINTER(C.c_uint32)] * 3
+        L.wlo_normal_pair.restype = None
+        L.wlo_normal_pair.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, _dp, _dp]
+        L.wlo_generate_loops.restype = C.c_int
+        L.wlo_generate_loops.argtypes = [C.c_uint64, C.c_int64, C.c_int64, C.c_int, _dp]
+        L.wlo_num_threads.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(_dp) if a is not None else None
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def field_g(profile, params, rho):
+    """g(rho) = e A_phi(rho)/rho, vectorised over rho."""
+    pr = _f64(params)
+    r = np.atleast_1d(_f64(rho))
+    return np.array([lib().wlo_field_g(profile, _p(pr), float(x)) for x in r.ravel()]).reshape(r.shape)
+
+
+def field_b(profile, params, rho):
+    """b(rho) = e B_z(rho), vectorised over rho."""
+    pr = _f64(params)
+    r = np.atleast_1d(_f64(rho))
+    return np.array([lib().wlo_field_b(profile, _p(pr), float(x)) for x in r.ravel()]).reshape(r.shape)
+
+
+def loop_phase_spin(profile, params, y, T, cx, cy):
+    """(phase, spin) of one unit loop y[N][2] at proper time T and centre (cx, cy)."""
+    pr = _f64(params)
+    y = _f64(y)
+    assert y.ndim == 2 and y.shape[1] == 2
+    ph, sp = C.c_double(), C.c_double()
+    lib().wlo_loop_phase_spin(profile, _p(pr), _p(y), y.shape[0], float(T), float(cx), float(cy),
+                              C.byref(ph), C.byref(sp))
+    return ph.value, sp.value
+
+
+def evaluate(profile, params, loops, T, rho_cm, phi_cm=None, n_groups=1, per_loop=False):
+    """Whole-ensemble evaluation.
+
+    loops [n_loops][N][2] (float32 storage is promoted exactly to float64).
+    Returns dict(W_mean [n_T][n_rho], group_sums [G][n_T][n_rho]) and, if per_loop,
+    W, phase, spin of shape [n_loops][n_T][n_rho].
+    """
+    pr = _f64(params)
+    y = _f64(loops)
+    assert y.ndim == 3 and y.shape[2] == 2
+    T = _f64(T)
+    rho = _f64(rho_cm)
+    phi = _f64(phi_cm) if phi_cm is not None else None
+    nl, N = y.shape[0], y.shape[1]
+    nT, nr = T.shape[0], rho.shape[0]
+    if phi is not None:
+        assert phi.shape == rho.shape
+    mean = np.empty((nT, nr))
+    gs = np.empty((n_groups, nT, nr))
+    W = ph = sp = None
+    if per_loop:
+        W, ph, sp = (np.empty((nl, nT, nr)) for _ in range(3))
+    rc = lib().wlo_eval(profile, _p(pr), _p(y), nl, N, _p(T), nT, _p(rho), _p(phi), nr, n_groups,
+                        _p(mean), _p(gs), _p(W), _p(ph), _p(sp))
+    if rc != 0:
+        raise ValueError("wlo_eval: invalid argument")
+    out = {"W_mean": mean, "group_sums": gs}
+    if per_loop:
+        out.update(W=W, phase=ph, spin=sp)
+    return out
+
+
+def finalize(group_sums, n_loops, delete_one=False):
+    """eq. (60)-(63): (mean, err[, delete-one-group means]) from group sums [G][...]."""
+    gs = _f64(group_sums)
+    G = gs.shape[0]
+    grid_shape = gs.shape[1:]
+    n_grid = int(np.prod(grid_shape)) if grid_shape else 1
+    mean = np.empty(n_grid)
+    err = np.empty(n_grid)
+    d1 = np.empty((G, n_grid)) if delete_one else None
+    rc = lib().wlo_finalize(_p(gs), G, n_loops, n_grid, _p(mean), _p(err), _p(d1))
+    if rc != 0:
+        raise ValueError("wlo_finalize: invalid argument")
+    res = (mean.reshape(grid_shape), err.reshape(grid_shape))
+    if delete_one:
+        res += (d1.reshape((G,) + grid_shape),)
+    return res
+
+
+def philox4x32_10(ctr, key):
+    c = (C.c_uint32 * 4)(*[int(x) for x in ctr])
+    k = (C.c_uint32 * 2)(*[int(x) for x in key])
+    o = (C.c_uint32 * 4)()
+    lib().wlo_philox4x32_10(c, k, o)
+    return [int(x) for x in o]
+
+
+def normal_pair(seed, loop, point):
+    a, b = C.c_double(), C.c_double()
+    lib().wlo_normal_pair(seed, loop, point, C.byref(a), C.byref(b))
+    return a.value, b.value
+
+
+def generate_loops(seed, n_loops, n_ppl, loop_begin=0):
+    """Unit d-loops [n_loops][n_ppl][2], FP64, centre of mass at the origin."""
+    out = np.empty((n_loops, n_ppl, 2))
+    rc = lib().wlo_generate_loops(seed, loop_begin, n_loops, n_ppl, _p(out))
+    if rc != 0:
+        raise ValueError("wlo_generate_loops: n_ppl must be a power of two >= 2")
+    return out
+
+
+def num_threads():
+    return lib().wlo_num_threads()
