@@ -1,0 +1,156 @@
+/*
+ * wl.h -- C ABI of the B200-native worldline-numerics hot path (libwl.so).
+ *
+ * Method: Mazur & Heyl, "Parallel Worldline Numerics: Implementation and Error
+ * Analysis", arXiv:1407.7486.  Citations are "PAPER.md:<line>" of the text of
+ * that paper plus its section / equation number.
+ *
+ * What the library computes (DESIGN.md section 1 has the full statement):
+ *   for every unit loop y_l (N points, 2-D), proper time T_t and centre of
+ *   mass x_cm,r = rho_r (cos phi_r, sin phi_r):
+ *     x_i   = x_cm + sqrt(T) y_i                                eq. (8),
+ *     phase = sum_i g(|m_i|) (m_i x d_i),  m_i = (x_i+x_{i+1})/2,
+ *             d_i = x_{i+1}-x_i, i+1 mod N, g = e A_phi/rho     eq. (21)-(24)
+ *     spin  = (T/N) sum_i e B(|x_i|)                            eq. (31)-(33)
+ *     W     = cos(phase) cosh(spin)                             eq. (18)
+ *   S_g = sum of W over the loops of jackknife group g          eq. (60)
+ *   <W> = (sum_g S_g)/N_l                                       eq. (61)-(62)
+ *   err = sqrt(sum_g (<W>_g - <W>)^2 / (G (G-1)))               eq. (63)
+ *
+ * Conventions
+ *   - "d_" pointers are DEVICE pointers, "h_" pointers are HOST pointers.
+ *   - The caller owns every buffer.  Except for wl_eval_host (which says so),
+ *     no call allocates device memory, synchronises the stream or the device,
+ *     or copies between host and device: all work is enqueued on `stream`.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default
+ *     stream), so that this header needs no CUDA header.
+ *   - All grids and results are FP64.  Loop coordinates are FP32 or FP64,
+ *     array-of-points: loops[l][i][c], c = 0 (x), 1 (y), contiguous.
+ *   - Every call returns a wl_status; nothing is printed, nothing aborts.
+ *     On any status other than WL_OK no kernel has been launched by that call.
+ *     (The paper's convention is "check the code, print the string",
+ *     PAPER.md:603-628; wl_status_string gives the string.)
+ *   - There is no CPU fallback: without a CUDA device the compute calls
+ *     return WL_ERR_CUDA.
+ */
+#ifndef WL_H
+#define WL_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    WL_OK = 0,
+    WL_ERR_INVALID_ARG = 1,   /* null pointer, bad size, bad parameter value     */
+    WL_ERR_UNSUPPORTED = 2,   /* valid request this build has no kernel for      */
+    WL_ERR_WORKSPACE = 3,     /* workspace null or smaller than *_workspace_bytes */
+    WL_ERR_CUDA = 4           /* a CUDA runtime call failed (no device, launch)  */
+} wl_status;
+
+/* Field profiles B_z(rho), gauge A = A_phi(rho) e_phi, A_phi = Phi(rho)/(2 pi rho)
+ * (eq. (13)-(17)).  The charge e is folded into the strength. */
+typedef enum {
+    WL_PROFILE_UNIFORM = 0,   /* params {eB}:           B_z = B, A = (B/2)(-y, x)            */
+    WL_PROFILE_SECH2 = 1      /* params {eB0, lambda}:  B_z = B0 sech^2(rho/lambda),
+                                 Phi = 2 pi B0 [lambda rho tanh(rho/lambda)
+                                               - lambda^2 ln cosh(rho/lambda)]               */
+} wl_profile;
+
+typedef enum { WL_F32 = 0, WL_F64 = 1 } wl_dtype;
+
+typedef struct wl_field wl_field;   /* opaque, host memory, immutable after creation */
+
+/* Creates a field description.  h_params: UNIFORM n_params == 1 {eB};
+ * SECH2 n_params == 2 {eB0, lambda}, lambda > 0.  Non-finite values, lambda <= 0,
+ * a wrong n_params or an unknown profile give WL_ERR_INVALID_ARG and *out = NULL.
+ * The caller releases it with wl_field_destroy.  Host-only; no CUDA call. */
+wl_status wl_field_create(wl_profile profile, const double* h_params, int n_params, wl_field** out);
+void wl_field_destroy(wl_field* field);   /* NULL is allowed */
+
+/* Seeded unit-loop ensemble: d-loops, steps (1)-(5), eq. (10)-(11), PAPER.md:65-81,
+ * centre of mass shifted to the origin, driven by Philox4x32-10 with counter
+ * (point, loop_lo, loop_hi, 0) and key (seed_lo, seed_hi) (reading A11).
+ * Writes loops [loop_begin, loop_begin + n_loops) of the ensemble `seed` to
+ * d_loops[n_loops][n_ppl][2] in `storage` precision (arithmetic is FP64; FP32
+ * storage rounds once at the store).  Loop l of an ensemble is the same whatever
+ * loop_begin / n_loops window it is generated in.
+ * n_ppl: power of two, 2 <= n_ppl <= 8192.  n_loops == 0 is a no-op.  */
+wl_status wl_loops_generate(void* d_loops, wl_dtype storage, int64_t loop_begin, int64_t n_loops,
+                            int n_ppl, uint64_t seed, void* stream);
+
+/* Bytes of device workspace wl_eval needs for these sizes (0 on invalid sizes).
+ * The workspace holds per-loop-chunk partial sums; its contents are scratch. */
+size_t wl_eval_workspace_bytes(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups,
+                               wl_dtype compute);
+
+/* The hot path.  For every (T_t, rho_r[, phi_r]) evaluates W for all loops and
+ * reduces them, in a fixed order that depends only on the argument sizes:
+ *   d_W_mean[t][r]        = <W>                    (n_T x n_rho, FP64)
+ *   d_group_sums[g][t][r] = S_g, group g = loops [g n_loops/G, (g+1) n_loops/G)
+ * d_loops [n_loops][n_ppl][2] of loop_dtype; n_ppl >= 1 (any value, not only
+ * powers of two).  d_T[n_T] > 0; d_rho_cm[n_rho] >= 0; d_phi_cm[n_rho] or NULL
+ * (= all zero).  Grid VALUES are not read on the host and are not validated.
+ * compute = WL_F64: all arithmetic FP64.  compute = WL_F32: per-term arithmetic
+ * FP32 with fast intrinsics, the sums round a loop accumulated in FP64 from
+ * FP32 partials of 32 terms, cos/cosh and all sums over loops FP64.
+ * Errors: null pointers, sizes < 1, n_groups < 1, n_loops % n_groups != 0
+ * (equal groups are required) -> WL_ERR_INVALID_ARG; workspace
+ * too small -> WL_ERR_WORKSPACE. */
+wl_status wl_eval(const wl_field* field,
+                  const void* d_loops, wl_dtype loop_dtype, int64_t n_loops, int n_ppl,
+                  const double* d_T, int n_T,
+                  const double* d_rho_cm, const double* d_phi_cm, int n_rho,
+                  int n_groups, wl_dtype compute,
+                  double* d_W_mean, double* d_group_sums,
+                  void* d_workspace, size_t workspace_bytes, void* stream);
+
+/* Same kernels, but the per-loop values are written instead of reduced (for
+ * parity triage; not part of the timed path):  d_W, d_phase, d_spin are each
+ * [n_loops][n_T][n_rho] FP64; d_phase / d_spin may be NULL.  No workspace. */
+wl_status wl_eval_per_loop(const wl_field* field,
+                           const void* d_loops, wl_dtype loop_dtype, int64_t n_loops, int n_ppl,
+                           const double* d_T, int n_T,
+                           const double* d_rho_cm, const double* d_phi_cm, int n_rho,
+                           wl_dtype compute,
+                           double* d_W, double* d_phase, double* d_spin, void* stream);
+
+/* Jackknife finalise, eq. (60)-(63).  From d_group_sums[G][n_T][n_rho]:
+ *   d_mean[t][r] = (sum_g S_g)/n_loops,
+ *   d_err[t][r]  = sqrt(sum_g (S_g G/n_loops - mean)^2 / (G (G-1))),
+ *   d_delete_one[g][t][r] = (sum_g' S_g' - S_g)/(n_loops - n_loops/G)   (NULL = skip).
+ * n_groups >= 2 and n_loops % n_groups == 0, else WL_ERR_INVALID_ARG. */
+wl_status wl_jackknife_finalize(const double* d_group_sums, int n_groups, int64_t n_loops,
+                                int n_T, int n_rho,
+                                double* d_mean, double* d_err, double* d_delete_one, void* stream);
+
+/* End-to-end convenience call on HOST buffers: allocates device memory, copies
+ * h_loops / grids to the device, runs wl_eval + wl_jackknife_finalize on an
+ * internal stream, copies h_W_mean[n_T][n_rho], h_err[n_T][n_rho] and
+ * h_group_sums[G][n_T][n_rho] back, frees the device memory and returns after
+ * everything has completed.  h_phi_cm, h_err and h_group_sums may be NULL.
+ * This is the only call that allocates, copies and synchronises. */
+wl_status wl_eval_host(const wl_field* field,
+                       const void* h_loops, wl_dtype loop_dtype, int64_t n_loops, int n_ppl,
+                       const double* h_T, int n_T,
+                       const double* h_rho_cm, const double* h_phi_cm, int n_rho,
+                       int n_groups, wl_dtype compute,
+                       double* h_W_mean, double* h_err, double* h_group_sums);
+
+/* Number of kernels wl_eval enqueues for these sizes (for launch accounting). */
+int wl_eval_launch_count(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups,
+                         wl_dtype compute);
+
+/* Static string for a status code (never NULL). */
+const char* wl_status_string(wl_status status);
+
+/* "major.minor" of this ABI. */
+const char* wl_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WL_H */

@@ -1,0 +1,242 @@
+"""Thin Python binding of libwl.so (include/wl.h): argument marshalling only.
+
+Every function has the name of the C entry point it calls.  Tensors are PyTorch CUDA tensors
+(device memory and streams are PyTorch's; all arithmetic runs in the library's kernels).
+There is no CPU fallback: importing this module raises if libwl.so is missing or does not
+load, and each call raises WLError on a non-zero status.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libwl.so")
+
+WL_OK = 0
+PROFILE_UNIFORM = 0
+PROFILE_SECH2 = 1
+F32 = 0
+F64 = 1
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError("%s not found: build it with `python -m paper_1407_7486_b200.build` "
+                      "(there is no CPU fallback)" % LIB_PATH)
+_lib = C.CDLL(LIB_PATH)
+
+_vp, _dp, _i64, _int, _u64, _sz = C.c_void_p, C.c_void_p, C.c_int64, C.c_int, C.c_uint64, C.c_size_t
+_lib.wl_field_create.restype = _int
+_lib.wl_field_create.argtypes = [_int, C.POINTER(C.c_double), _int, C.POINTER(_vp)]
+_lib.wl_field_destroy.restype = None
+_lib.wl_field_destroy.argtypes = [_vp]
+_lib.wl_loops_generate.restype = _int
+_lib.wl_loops_generate.argtypes = [_vp, _int, _i64, _i64, _int, _u64, _vp]
+_lib.wl_eval_workspace_bytes.restype = _sz
+_lib.wl_eval_workspace_bytes.argtypes = [_i64, _int, _int, _int, _int, _int]
+_lib.wl_eval_launch_count.restype = _int
+_lib.wl_eval_launch_count.argtypes = [_i64, _int, _int, _int, _int, _int]
+_lib.wl_eval.restype = _int
+_lib.wl_eval.argtypes = [_vp, _vp, _int, _i64, _int, _dp, _int, _dp, _dp, _int, _int, _int, _dp, _dp,
+                         _vp, _sz, _vp]
+_lib.wl_eval_per_loop.restype = _int
+_lib.wl_eval_per_loop.argtypes = [_vp, _vp, _int, _i64, _int, _dp, _int, _dp, _dp, _int, _int, _dp, _dp,
+                                  _dp, _vp]
+_lib.wl_jackknife_finalize.restype = _int
+_lib.wl_jackknife_finalize.argtypes = [_dp, _int, _i64, _int, _int, _dp, _dp, _dp, _vp]
+_lib.wl_eval_host.restype = _int
+_lib.wl_eval_host.argtypes = [_vp, _vp, _int, _i64, _int, _dp, _int, _dp, _dp, _int, _int, _int, _dp, _dp,
+                              _dp]
+_lib.wl_status_string.restype = C.c_char_p
+_lib.wl_status_string.argtypes = [_int]
+_lib.wl_version.restype = C.c_char_p
+_lib.wl_version.argtypes = []
+
+
+class WLError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = int(status)
+        super().__init__("%s: %s (status %d)" % (where, wl_status_string(status), status))
+
+
+def _check(status, where):
+    if status != WL_OK:
+        raise WLError(status, where)
+
+
+def wl_status_string(status) -> str:
+    return _lib.wl_status_string(int(status)).decode()
+
+
+def wl_version() -> str:
+    return _lib.wl_version().decode()
+
+
+def _dtype_code(dt) -> int:
+    if isinstance(dt, int) and not isinstance(dt, bool) and dt in (F32, F64):
+        return dt
+    s = str(dt)
+    if "float32" in s or s == "f32":
+        return F32
+    if "float64" in s or s == "f64":
+        return F64
+    raise ValueError("dtype must be float32 or float64, got %r" % (dt,))
+
+
+def _stream(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+def _cuda_f64(t, name, numel=None):
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise ValueError("%s must be a contiguous float64 CUDA tensor" % name)
+    if numel is not None and t.numel() != numel:
+        raise ValueError("%s must have %d elements" % (name, numel))
+    return t
+
+
+def _ptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else None
+
+
+class Field:
+    """Owns a wl_field* (wl_field_create / wl_field_destroy)."""
+
+    def __init__(self, profile, params):
+        arr = (C.c_double * len(params))(*[float(p) for p in params])
+        h = C.c_void_p()
+        _check(_lib.wl_field_create(int(profile), arr, len(params), C.byref(h)), "wl_field_create")
+        self._h = h
+        self.profile = int(profile)
+        self.params = tuple(float(p) for p in params)
+
+    def __del__(self, _destroy=_lib.wl_field_destroy):
+        h, self._h = getattr(self, "_h", None), None
+        if h:
+            _destroy(h)
+
+
+def wl_field_create(profile, params) -> Field:
+    return Field(profile, params)
+
+
+def wl_loops_generate(n_loops, n_ppl, seed, dtype=torch.float64, loop_begin=0, out=None, device="cuda",
+                      stream=None) -> torch.Tensor:
+    """Unit d-loops [n_loops][n_ppl][2] of ensemble `seed`, loops loop_begin .. loop_begin+n_loops-1."""
+    if out is None:
+        out = torch.empty((n_loops, n_ppl, 2), dtype=dtype, device=device)
+    if not (out.is_cuda and out.is_contiguous() and out.shape == (n_loops, n_ppl, 2)):
+        raise ValueError("out must be a contiguous CUDA tensor [n_loops][n_ppl][2]")
+    with torch.cuda.device(out.device):
+        _check(_lib.wl_loops_generate(_ptr(out), _dtype_code(out.dtype), int(loop_begin), int(n_loops),
+                                      int(n_ppl), int(seed), _stream(stream)), "wl_loops_generate")
+    return out
+
+
+def wl_eval_workspace_bytes(n_loops, n_ppl, n_T, n_rho, n_groups, compute) -> int:
+    return int(_lib.wl_eval_workspace_bytes(n_loops, n_ppl, n_T, n_rho, n_groups, _dtype_code(compute)))
+
+
+def wl_eval_launch_count(n_loops, n_ppl, n_T, n_rho, n_groups, compute) -> int:
+    return int(_lib.wl_eval_launch_count(n_loops, n_ppl, n_T, n_rho, n_groups, _dtype_code(compute)))
+
+
+def _loops_arg(loops):
+    if not (isinstance(loops, torch.Tensor) and loops.is_cuda and loops.is_contiguous() and loops.dim() == 3
+            and loops.shape[2] == 2 and loops.dtype in (torch.float32, torch.float64)):
+        raise ValueError("loops must be a contiguous CUDA tensor [n_loops][n_ppl][2], float32 or float64")
+    return loops.shape[0], loops.shape[1]
+
+
+def wl_eval(field, loops, T, rho_cm, phi_cm=None, n_groups=1, compute=torch.float64, W_mean=None,
+            group_sums=None, workspace=None, stream=None):
+    """Returns (W_mean [n_T][n_rho], group_sums [G][n_T][n_rho]); see include/wl.h."""
+    n_loops, n_ppl = _loops_arg(loops)
+    T = _cuda_f64(T, "T")
+    rho_cm = _cuda_f64(rho_cm, "rho_cm")
+    n_T, n_rho = T.numel(), rho_cm.numel()
+    phi_cm = _cuda_f64(phi_cm, "phi_cm", n_rho)
+    dev = loops.device
+    if W_mean is None:
+        W_mean = torch.empty((n_T, n_rho), dtype=torch.float64, device=dev)
+    if group_sums is None:
+        group_sums = torch.empty((n_groups, n_T, n_rho), dtype=torch.float64, device=dev)
+    _cuda_f64(W_mean, "W_mean", n_T * n_rho)
+    _cuda_f64(group_sums, "group_sums", n_groups * n_T * n_rho)
+    cc = _dtype_code(compute)
+    if workspace is None:
+        need = int(_lib.wl_eval_workspace_bytes(n_loops, n_ppl, n_T, n_rho, n_groups, cc))
+        workspace = torch.empty(max(need, 8), dtype=torch.uint8, device=dev)
+    with torch.cuda.device(dev):
+        _check(_lib.wl_eval(field._h, _ptr(loops), _dtype_code(loops.dtype), n_loops, n_ppl, _ptr(T), n_T,
+                            _ptr(rho_cm), _ptr(phi_cm), n_rho, int(n_groups), cc, _ptr(W_mean),
+                            _ptr(group_sums), _ptr(workspace), workspace.numel() * workspace.element_size(),
+                            _stream(stream)), "wl_eval")
+    return W_mean, group_sums
+
+
+def wl_eval_per_loop(field, loops, T, rho_cm, phi_cm=None, compute=torch.float64, want_phase_spin=True,
+                     stream=None):
+    """Per-loop (W, phase, spin), each [n_loops][n_T][n_rho] (phase/spin None if not wanted)."""
+    n_loops, n_ppl = _loops_arg(loops)
+    T = _cuda_f64(T, "T")
+    rho_cm = _cuda_f64(rho_cm, "rho_cm")
+    n_T, n_rho = T.numel(), rho_cm.numel()
+    phi_cm = _cuda_f64(phi_cm, "phi_cm", n_rho)
+    dev = loops.device
+    W = torch.empty((n_loops, n_T, n_rho), dtype=torch.float64, device=dev)
+    ph = torch.empty_like(W) if want_phase_spin else None
+    sp = torch.empty_like(W) if want_phase_spin else None
+    with torch.cuda.device(dev):
+        _check(_lib.wl_eval_per_loop(field._h, _ptr(loops), _dtype_code(loops.dtype), n_loops, n_ppl, _ptr(T),
+                                     n_T, _ptr(rho_cm), _ptr(phi_cm), n_rho, _dtype_code(compute), _ptr(W),
+                                     _ptr(ph), _ptr(sp), _stream(stream)), "wl_eval_per_loop")
+    return W, ph, sp
+
+
+def wl_jackknife_finalize(group_sums, n_loops, delete_one=False, stream=None):
+    """(mean, err[, delete-one-group means]) from group_sums [G][n_T][n_rho]; eq. (60)-(63)."""
+    gs = _cuda_f64(group_sums, "group_sums")
+    if gs.dim() != 3:
+        raise ValueError("group_sums must be [G][n_T][n_rho]")
+    G, n_T, n_rho = gs.shape
+    mean = torch.empty((n_T, n_rho), dtype=torch.float64, device=gs.device)
+    err = torch.empty_like(mean)
+    d1 = torch.empty_like(gs) if delete_one else None
+    with torch.cuda.device(gs.device):
+        _check(_lib.wl_jackknife_finalize(_ptr(gs), G, int(n_loops), n_T, n_rho, _ptr(mean), _ptr(err),
+                                          _ptr(d1), _stream(stream)), "wl_jackknife_finalize")
+    return (mean, err, d1) if delete_one else (mean, err)
+
+
+def wl_eval_host(field, loops, T, rho_cm, phi_cm=None, n_groups=2, compute=torch.float64):
+    """End-to-end call on HOST buffers (numpy arrays or CPU tensors; pinned memory is used as given).
+
+    Returns numpy (W_mean, err, group_sums).  All copies happen inside the C call.
+    """
+    def host(a, dt=None):
+        if isinstance(a, torch.Tensor):
+            if a.is_cuda:
+                raise ValueError("wl_eval_host takes host buffers")
+            a = a.numpy()
+        a = np.ascontiguousarray(a) if dt is None else np.ascontiguousarray(a, dtype=dt)
+        return a
+    y = host(loops)
+    if y.dtype not in (np.float32, np.float64) or y.ndim != 3 or y.shape[2] != 2:
+        raise ValueError("loops must be [n_loops][n_ppl][2], float32 or float64")
+    T = host(T, np.float64)
+    rho = host(rho_cm, np.float64)
+    phi = host(phi_cm, np.float64) if phi_cm is not None else None
+    n_T, n_rho = T.size, rho.size
+    mean = np.empty((n_T, n_rho))
+    err = np.empty((n_T, n_rho))
+    gs = np.empty((n_groups, n_T, n_rho))
+    p = lambda a: C.c_void_p(a.ctypes.data) if a is not None else None
+    _check(_lib.wl_eval_host(field._h, p(y), _dtype_code(y.dtype.type), y.shape[0], y.shape[1], p(T), n_T,
+                             p(rho), p(phi), n_rho, int(n_groups), _dtype_code(compute), p(mean), p(err),
+                             p(gs)), "wl_eval_host")
+    return mean, err, gs

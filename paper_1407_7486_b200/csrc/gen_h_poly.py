@@ -1,0 +1,59 @@
+"""Prints the polynomial coefficients used by wl_field_device.cuh (CUDA path only).
+
+h(u) = [u tanh u - ln cosh u]/u^2 is even and analytic in w = u^2 for |w| < pi^2/4, so near
+the axis the kernels evaluate a polynomial in w instead of the closed form, whose
+subtraction loses digits as u -> 0.  This script interpolates h at
+Chebyshev nodes of [0, w_max] with mpmath (50 digits), converts to monomial coefficients
+in w and reports the maximum relative error on a fine grid.
+
+Usage:  python gen_h_poly.py <w_max> <degree>
+Not imported by anything; the printed numbers were pasted into wl_field_device.cuh.
+Independent of oracle/ (which uses the Maclaurin series for u < 0.1).
+"""
+import sys
+
+import mpmath as mp
+
+mp.mp.dps = 50
+
+
+def h(w):
+    w = mp.mpf(w)
+    if w == 0:
+        return mp.mpf(1) / 2
+    u = mp.sqrt(w)
+    return (u * mp.tanh(u) - mp.log(mp.cosh(u))) / w
+
+
+def fit(w_max, deg):
+    n = deg + 1
+    nodes = [(mp.cos(mp.pi * (2 * k + 1) / (2 * n)) + 1) / 2 * w_max for k in range(n)]
+    A = mp.matrix(n, n)
+    b = mp.matrix(n, 1)
+    for r, x in enumerate(nodes):
+        for c in range(n):
+            A[r, c] = x ** c
+        b[r] = h(x)
+    coef = mp.lu_solve(A, b)
+    return [coef[i] for i in range(n)]
+
+
+def max_rel_err(coef, w_max, cast):
+    worst = mp.mpf(0)
+    for k in range(2001):
+        w = mp.mpf(w_max) * k / 2000
+        acc = mp.mpf(0)
+        for c in reversed(coef):
+            acc = acc * w + cast(c)
+        worst = max(worst, abs(acc / h(w) - 1))
+    return worst
+
+
+if __name__ == "__main__":
+    w_max = float(sys.argv[1])
+    deg = int(sys.argv[2])
+    coef = fit(w_max, deg)
+    print("// h(w), w = u^2 in [0, %g], degree %d" % (w_max, deg))
+    print("// max rel. error (exact coefficients): %s" % mp.nstr(max_rel_err(coef, w_max, lambda c: c), 3))
+    for i, c in enumerate(coef):
+        print("c%d = %s" % (i, mp.nstr(c, 20)))

@@ -1,0 +1,145 @@
+// wl_api.cu -- the extern "C" entry points of include/wl.h: argument checks and launches only.
+#include <cmath>
+#include <new>
+
+#include "wl_internal.cuh"
+
+using namespace wl;
+
+namespace {
+
+bool sizes_ok(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups)
+{
+    if (n_loops < 1 || n_ppl < 1 || n_T < 1 || n_rho < 1 || n_groups < 1) return false;
+    if (n_loops % n_groups != 0) return false;                       // equal groups
+    if ((int64_t)n_T * n_rho > (1 << 24)) return false;
+    if (n_loops > (1LL << 40)) return false;
+    return true;
+}
+
+bool dtype_ok(wl_dtype d) { return d == WL_F32 || d == WL_F64; }
+
+}  // namespace
+
+extern "C" {
+
+wl_status wl_field_create(wl_profile profile, const double* h_params, int n_params, wl_field** out)
+{
+    if (!out) return WL_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!h_params) return WL_ERR_INVALID_ARG;
+    if (profile == WL_PROFILE_UNIFORM) {
+        if (n_params != 1 || !std::isfinite(h_params[0])) return WL_ERR_INVALID_ARG;
+    } else if (profile == WL_PROFILE_SECH2) {
+        if (n_params != 2 || !std::isfinite(h_params[0]) || !std::isfinite(h_params[1]) || !(h_params[1] > 0.0))
+            return WL_ERR_INVALID_ARG;
+    } else {
+        return WL_ERR_INVALID_ARG;
+    }
+    wl_field* f = new (std::nothrow) wl_field;
+    if (!f) return WL_ERR_INVALID_ARG;
+    f->profile = (int)profile;
+    f->p0 = h_params[0];
+    f->p1 = (n_params > 1) ? h_params[1] : 0.0;
+    *out = f;
+    return WL_OK;
+}
+
+void wl_field_destroy(wl_field* field) { delete field; }
+
+wl_status wl_loops_generate(void* d_loops, wl_dtype storage, int64_t loop_begin, int64_t n_loops, int n_ppl,
+                            uint64_t seed, void* stream)
+{
+    if (!dtype_ok(storage) || n_loops < 0 || loop_begin < 0) return WL_ERR_INVALID_ARG;
+    if (n_ppl < 2 || n_ppl > kMaxPpl || (n_ppl & (n_ppl - 1)) != 0) return WL_ERR_INVALID_ARG;
+    if (n_loops == 0) return WL_OK;
+    if (!d_loops) return WL_ERR_INVALID_ARG;
+    cudaError_t e = launch_generate(d_loops, storage == WL_F64, loop_begin, n_loops, n_ppl, seed,
+                                    (cudaStream_t)stream);
+    return e == cudaSuccess ? WL_OK : WL_ERR_CUDA;
+}
+
+size_t wl_eval_workspace_bytes(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups, wl_dtype compute)
+{
+    if (!sizes_ok(n_loops, n_ppl, n_T, n_rho, n_groups) || !dtype_ok(compute)) return 0;
+    const EvalPlan p = make_eval_plan(n_loops, n_ppl, n_T, n_rho, n_groups, compute, false);
+    return (size_t)p.n_units * (size_t)p.n_grid * sizeof(double);
+}
+
+int wl_eval_launch_count(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups, wl_dtype compute)
+{
+    if (!sizes_ok(n_loops, n_ppl, n_T, n_rho, n_groups) || !dtype_ok(compute)) return 0;
+    return 3;   // k_wilson, k_group_reduce, k_mean
+}
+
+wl_status wl_eval(const wl_field* field, const void* d_loops, wl_dtype loop_dtype, int64_t n_loops, int n_ppl,
+                  const double* d_T, int n_T, const double* d_rho_cm, const double* d_phi_cm, int n_rho,
+                  int n_groups, wl_dtype compute, double* d_W_mean, double* d_group_sums,
+                  void* d_workspace, size_t workspace_bytes, void* stream)
+{
+    if (!field || !d_loops || !d_T || !d_rho_cm || !d_W_mean || !d_group_sums) return WL_ERR_INVALID_ARG;
+    if (!dtype_ok(loop_dtype) || !dtype_ok(compute)) return WL_ERR_INVALID_ARG;
+    if (!sizes_ok(n_loops, n_ppl, n_T, n_rho, n_groups)) return WL_ERR_INVALID_ARG;
+    const EvalPlan plan = make_eval_plan(n_loops, n_ppl, n_T, n_rho, n_groups, compute, false);
+    const size_t need = (size_t)plan.n_units * (size_t)plan.n_grid * sizeof(double);
+    if (!d_workspace || workspace_bytes < need) return WL_ERR_WORKSPACE;
+
+    EvalArgs a;
+    a.loops = d_loops; a.loops_are_f64 = (loop_dtype == WL_F64); a.n_loops = n_loops; a.n_ppl = n_ppl;
+    a.T = d_T; a.rho = d_rho_cm; a.phi = d_phi_cm; a.n_T = n_T; a.n_rho = n_rho;
+    a.p0 = field->p0; a.p1 = field->p1;
+    a.partial = reinterpret_cast<double*>(d_workspace);
+    a.phase_out = nullptr; a.spin_out = nullptr;
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaError_t e = launch_wilson(plan, a, field->profile, compute, s);
+    if (e != cudaSuccess) return e == cudaErrorInvalidValue ? WL_ERR_UNSUPPORTED : WL_ERR_CUDA;
+    e = launch_group_reduce(a.partial, plan.n_units, plan.units_per_group, n_groups, plan.n_grid, n_loops,
+                            d_group_sums, d_W_mean, s);
+    return e == cudaSuccess ? WL_OK : WL_ERR_CUDA;
+}
+
+wl_status wl_eval_per_loop(const wl_field* field, const void* d_loops, wl_dtype loop_dtype, int64_t n_loops,
+                           int n_ppl, const double* d_T, int n_T, const double* d_rho_cm,
+                           const double* d_phi_cm, int n_rho, wl_dtype compute,
+                           double* d_W, double* d_phase, double* d_spin, void* stream)
+{
+    if (!field || !d_loops || !d_T || !d_rho_cm || !d_W) return WL_ERR_INVALID_ARG;
+    if (!dtype_ok(loop_dtype) || !dtype_ok(compute)) return WL_ERR_INVALID_ARG;
+    if (!sizes_ok(n_loops, n_ppl, n_T, n_rho, 1)) return WL_ERR_INVALID_ARG;
+    const EvalPlan plan = make_eval_plan(n_loops, n_ppl, n_T, n_rho, 1, compute, true);
+    EvalArgs a;
+    a.loops = d_loops; a.loops_are_f64 = (loop_dtype == WL_F64); a.n_loops = n_loops; a.n_ppl = n_ppl;
+    a.T = d_T; a.rho = d_rho_cm; a.phi = d_phi_cm; a.n_T = n_T; a.n_rho = n_rho;
+    a.p0 = field->p0; a.p1 = field->p1;
+    a.partial = d_W; a.phase_out = d_phase; a.spin_out = d_spin;
+    cudaError_t e = launch_wilson(plan, a, field->profile, compute, (cudaStream_t)stream);
+    if (e != cudaSuccess) return e == cudaErrorInvalidValue ? WL_ERR_UNSUPPORTED : WL_ERR_CUDA;
+    return WL_OK;
+}
+
+wl_status wl_jackknife_finalize(const double* d_group_sums, int n_groups, int64_t n_loops, int n_T, int n_rho,
+                                double* d_mean, double* d_err, double* d_delete_one, void* stream)
+{
+    if (!d_group_sums || !d_mean || !d_err) return WL_ERR_INVALID_ARG;
+    if (n_groups < 2 || n_loops < 1 || n_loops % n_groups != 0 || n_T < 1 || n_rho < 1) return WL_ERR_INVALID_ARG;
+    if ((int64_t)n_T * n_rho > (1 << 24)) return WL_ERR_INVALID_ARG;
+    cudaError_t e = launch_finalize(d_group_sums, n_groups, n_loops, n_T * n_rho, d_mean, d_err, d_delete_one,
+                                    (cudaStream_t)stream);
+    return e == cudaSuccess ? WL_OK : WL_ERR_CUDA;
+}
+
+const char* wl_status_string(wl_status status)
+{
+    switch (status) {
+        case WL_OK: return "ok";
+        case WL_ERR_INVALID_ARG: return "invalid argument";
+        case WL_ERR_UNSUPPORTED: return "unsupported configuration";
+        case WL_ERR_WORKSPACE: return "workspace missing or too small";
+        case WL_ERR_CUDA: return "CUDA runtime error";
+    }
+    return "unknown status";
+}
+
+const char* wl_version(void) { return "1.0"; }
+
+}  // extern "C"
