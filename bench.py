@@ -1,0 +1,262 @@
+#!/usr/bin/env python
+"""bench.py -- Wilson-loop point-evals/s on the paper-scale ensemble (BASELINE.json config 3).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload 3]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 \
+           --master-port P bench.py --gpus N --steps K --warmup W
+
+One "step" = one pass of the whole hot path over one ensemble:
+wl_eval (k_wilson + k_group_reduce + k_mean) -> [N > 1: all-gather of the group sums] ->
+wl_jackknife_finalize.  metric = N_l * N_ppl * N_T * N_rho / time (loop-point evaluations per second).
+
+  value     : loops resident in HBM, timed on the device with CUDA events, max over ranks.
+  e2e       : the same step through the C-ABI call on HOST buffers (wl_eval_host: pinned host loops
+              -> device, kernels, results -> host inside the timed region).
+  roofline  : the dominant kernel (k_wilson) against the FP32 non-tensor issue roofline (DESIGN.md
+              section 5): achieved = 36 algorithmic lane-ops per point-eval x point-evals / kernel time.
+  cpu_baseline : the FP64 oracle (oracle/wl_oracle.c, as it stands) on a bounded sample, host cores.
+  --impl reference : times the oracle alone (this tier's reference arm); needs no GPU.
+
+Multi-GPU (weak scaling): every rank holds its own 16384 loops of one N x 16384-loop ensemble
+(whole jackknife groups per rank, paper_1407_7486_b200/shard.py); the only exchange is one all-gather
+of the group sums per step.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "wilson_loop_point_evals_per_s"
+UNIT = "point-evals/s"
+
+# algorithmic work per point-eval of the sech^2 profile in FP32
+# (SURVEY.md section 8(d)): 29 plain FP32 lane-ops + 7 special-function lane-ops.
+ALG_PLAIN_OPS = 29
+ALG_SFU_OPS = 7
+ALG_OPS_UNIFORM = 4
+SM_COUNT = 148
+ISSUE_LANES_PER_CLK_SM = 128      # 4 sub-partitions x 1 warp instruction (32 lanes) per clock
+FP64_LANES_PER_CLK_SM = 64        # measured 63.8 (profiles/r01_pipe_rates.md)
+SFU_LANES_PER_CLK_SM = 16         # measured 15.96
+
+
+def affinity_cores():
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons of one GPU through NVML while the timed region runs."""
+
+    def __init__(self, index, period=0.02):
+        super().__init__(daemon=True)
+        self.period = period
+        self.samples, self.reasons = [], set()
+        self.max_mhz = None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksThrottleReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake_slowdown",
+        }
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop_evt.wait(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2.0)
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+def nvml_index_for(device_index):
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+    if vis:
+        try:
+            return int(vis.split(",")[device_index])
+        except (ValueError, IndexError):
+            pass
+    return device_index
+
+
+def oracle_sample_loops(cfg, cores, per_four_cores):
+    """Whole-loop sample size for the oracle legs: `per_four_cores` loops per 4 host cores."""
+    n = per_four_cores * max(1, cores // 4)
+    return max(1, min(cfg.n_loops, n))
+
+
+def time_oracle(cfg, loops_host, T, rho, phi):
+    from oracle import wl_oracle as oracle
+    n = loops_host.shape[0]
+    G = 1
+    t0 = time.perf_counter()
+    oracle.evaluate(cfg.profile, cfg.params, loops_host, T, rho, phi, n_groups=G)
+    dt = time.perf_counter() - t0
+    evals = n * cfg.n_ppl * len(T) * len(rho)
+    return evals / dt, dt, oracle.num_threads()
+
+
+def base_line(args, cfg, n_gpus):
+    return {
+        "metric": METRIC, "unit": UNIT, "n_gpus": n_gpus, "steps": args.steps, "warmup": args.warmup,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "data": "synthetic",
+    }
+
+
+def workload_config(cfg, n_gpus, compute):
+    return {
+        "workload": cfg.name,
+        "n_loops_per_gpu": cfg.n_loops, "n_loops_total": cfg.n_loops * n_gpus, "n_ppl": cfg.n_ppl,
+        "n_T": cfg.n_T, "n_rho": cfg.n_rho, "n_groups_total": cfg.n_groups * n_gpus,
+        "field": {"profile": "sech2" if cfg.profile == 1 else "uniform", "params": list(cfg.params)},
+        "loop_storage": cfg.loop_dtype, "compute": compute, "seed": cfg.seed,
+        "parallelism": "dp%d (whole jackknife groups per rank)" % n_gpus,
+        "cache": "inputs larger than L2 (%.0f MB of loop coordinates per step vs 126 MB L2)"
+                 % (cfg.n_loops * cfg.n_ppl * 2 * (4 if cfg.loop_dtype == "f32" else 8) / 1e6),
+    }
+
+
+def run_reference(args, cfg):
+    """This tier's reference arm: the oracle, as it stands, on the host cores; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    import numpy as np
+    from oracle import wl_oracle as oracle
+    cores = affinity_cores()
+    n = oracle_sample_loops(cfg, cores, 64)
+    T, rho, phi = cfg.grids()
+    loops = oracle.generate_loops(cfg.seed, n, cfg.n_ppl)
+    if cfg.loop_dtype == "f32":
+        loops = loops.astype(np.float32).astype(np.float64)       # the stored coordinates, promoted exactly
+    for _ in range(args.warmup):
+        time_oracle(cfg, loops, T, rho, phi)
+    total_t, total_e, threads = 0.0, 0, 1
+    for _ in range(args.steps):
+        rate, dt, threads = time_oracle(cfg, loops, T, rho, phi)
+        total_t += dt
+        total_e += n * cfg.n_ppl * cfg.n_T * cfg.n_rho
+    value = total_e / total_t
+    sample = "%d whole loops x full %dx%d grid per step (of %d loops)" % (n, cfg.n_T, cfg.n_rho, cfg.n_loops)
+    line = base_line(args, cfg, args.gpus)
+    line.update({
+        "impl": "reference", "value": value, "ms_per_step": 1e3 * total_t / args.steps, "dtype": "f64",
+        "config": workload_config(cfg, 1, "f64 (oracle)"),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0, "scaling": "weak",
+    })
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def run_ours(args, cfg):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    from paper_1407_7486_b200 import api, shard        # raises if libwl.so is missing
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        if world == 1 and args.gpus > 1:
+            raise SystemExit("bench.py --gpus %d must be launched with torch.distributed.run (one rank per GPU)"
+                             % args.gpus)
+        raise SystemExit("WORLD_SIZE %d != --gpus %d" % (world, args.gpus))
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    compute = args.compute or ("f32" if "f32" in cfg.compute else "f64")
+    T, rho, phi = cfg.grids()
+    dev = lambda a: torch.tensor(a, dtype=torch.float64, device="cuda") if a is not None else None
+    Td, rd, pd = dev(T), dev(rho), dev(phi)
+    field = api.wl_field_create(cfg.profile, cfg.params)
+    sh = shard.shard_groups(cfg.n_loops * world, cfg.n_groups * world, world, rank)
+    tdt = torch.float32 if cfg.loop_dtype == "f32" else torch.float64
+    loops = api.wl_loops_generate(sh.n_loops, cfg.n_ppl, cfg.seed, tdt, loop_begin=sh.loop_begin)
+    ws_bytes = api.wl_eval_workspace_bytes(sh.n_loops, cfg.n_ppl, cfg.n_T, cfg.n_rho, sh.n_groups, compute)
+    workspace = torch.empty(max(ws_bytes, 8), dtype=torch.uint8, device="cuda")
+    W_mean = torch.empty((cfg.n_T, cfg.n_rho), dtype=torch.float64, device="cuda")
+    gs_local = torch.empty((sh.n_groups, cfg.n_T, cfg.n_rho), dtype=torch.float64, device="cuda")
+    n_loops_total = sh.n_loops * world
+    stream = torch.cuda.current_stream()
+
+    def step(events=None):
+        api.wl_eval(field, loops, Td, rd, pd, n_groups=sh.n_groups, compute=compute, W_mean=W_mean,
+                    group_sums=gs_local, workspace=workspace, wilson_events=events)
+        gs = shard.all_gather_group_sums(gs_local, world) if world > 1 else gs_local
+        return api.wl_jackknife_finalize(gs, n_loops_total)
+
+    def fence():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    fence()
+    k_events = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+                for _ in range(args.steps)]
+    for a, b in k_events:            # create the cudaEvent_t handles outside the timed region
+        a.record(stream)
+        b.record(stream)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(nvml_index_for(local_rank))
+    fence()
+    sampler.start()
+    e0.record(stream)
+    for k in range(args.steps):
+        mean, err = step(k_events[k])
+    e1.record(stream)
+    fence()
+    clocks = sampler.stop()
+    ms_total = e0.elapsed_time(e1)
+    wilson_ms = [a.elapsed_time(b) for a, b in k_events]
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_per_step = ms_total / args.steps
+    evals_per_gpu = cfg.point_evals
+    value = evals_per_gpu * world / (ms_per_step * 1e-3)
+    result_checksum = float(mean.sum().item())
+    if not np.isfinite(result_checksum):
+        raise SystemExit("bench.py: non-finite <W>")

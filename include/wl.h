@@ -108,6 +108,19 @@ wl_status wl_eval(const wl_field* field,
                   double* d_W_mean, double* d_group_sums,
                   void* d_workspace, size_t workspace_bytes, void* stream);
 
+/* wl_eval with two optional CUDA events (cudaEvent_t passed as void*, NULL = none)
+ * recorded on `stream` immediately before and after the k_wilson launch, so that a
+ * benchmark can time the dominant kernel alone inside the step (SURVEY.md section 8(d):
+ * a2+a3 are > 99.9 % of the work).  Everything else is exactly wl_eval. */
+wl_status wl_eval_instrumented(const wl_field* field,
+                  const void* d_loops, wl_dtype loop_dtype, int64_t n_loops, int n_ppl,
+                  const double* d_T, int n_T,
+                  const double* d_rho_cm, const double* d_phi_cm, int n_rho,
+                  int n_groups, wl_dtype compute,
+                  double* d_W_mean, double* d_group_sums,
+                  void* d_workspace, size_t workspace_bytes, void* stream,
+                  void* event_wilson_begin, void* event_wilson_end);
+
 /* Same kernels, but the per-loop values are written instead of reduced (for
  * parity triage; not part of the timed path):  d_W, d_phase, d_spin are each
  * [n_loops][n_T][n_rho] FP64; d_phase / d_spin may be NULL.  No workspace. */

@@ -39,6 +39,8 @@ _lib.wl_eval_launch_count.argtypes = [_i64, _int, _int, _int, _int, _int]
 _lib.wl_eval.restype = _int
 _lib.wl_eval.argtypes = [_vp, _vp, _int, _i64, _int, _dp, _int, _dp, _dp, _int, _int, _int, _dp, _dp,
                          _vp, _sz, _vp]
+_lib.wl_eval_instrumented.restype = _int
+_lib.wl_eval_instrumented.argtypes = list(_lib.wl_eval.argtypes) + [_vp, _vp]
 _lib.wl_eval_per_loop.restype = _int
 _lib.wl_eval_per_loop.argtypes = [_vp, _vp, _int, _i64, _int, _dp, _int, _dp, _dp, _int, _int, _dp, _dp,
                                   _dp, _vp]
@@ -152,9 +154,20 @@ def _loops_arg(loops):
     return loops.shape[0], loops.shape[1]
 
 
+def _event_handle(ev, stream):
+    if ev is None:
+        return None
+    if not ev.cuda_event:          # torch creates the cudaEvent_t lazily, on the first record()
+        ev.record(stream if stream is not None else torch.cuda.current_stream())
+    return C.c_void_p(ev.cuda_event)
+
+
 def wl_eval(field, loops, T, rho_cm, phi_cm=None, n_groups=1, compute=torch.float64, W_mean=None,
-            group_sums=None, workspace=None, stream=None):
-    """Returns (W_mean [n_T][n_rho], group_sums [G][n_T][n_rho]); see include/wl.h."""
+            group_sums=None, workspace=None, stream=None, wilson_events=None):
+    """Returns (W_mean [n_T][n_rho], group_sums [G][n_T][n_rho]); see include/wl.h.
+
+    wilson_events = (begin, end) torch.cuda.Event pair (enable_timing=True): calls
+    wl_eval_instrumented, which records them around the k_wilson launch."""
     n_loops, n_ppl = _loops_arg(loops)
     T = _cuda_f64(T, "T")
     rho_cm = _cuda_f64(rho_cm, "rho_cm")
@@ -171,11 +184,15 @@ def wl_eval(field, loops, T, rho_cm, phi_cm=None, n_groups=1, compute=torch.floa
     if workspace is None:
         need = int(_lib.wl_eval_workspace_bytes(n_loops, n_ppl, n_T, n_rho, n_groups, cc))
         workspace = torch.empty(max(need, 8), dtype=torch.uint8, device=dev)
+    args = (field._h, _ptr(loops), _dtype_code(loops.dtype), n_loops, n_ppl, _ptr(T), n_T,
+            _ptr(rho_cm), _ptr(phi_cm), n_rho, int(n_groups), cc, _ptr(W_mean),
+            _ptr(group_sums), _ptr(workspace), workspace.numel() * workspace.element_size())
     with torch.cuda.device(dev):
-        _check(_lib.wl_eval(field._h, _ptr(loops), _dtype_code(loops.dtype), n_loops, n_ppl, _ptr(T), n_T,
-                            _ptr(rho_cm), _ptr(phi_cm), n_rho, int(n_groups), cc, _ptr(W_mean),
-                            _ptr(group_sums), _ptr(workspace), workspace.numel() * workspace.element_size(),
-                            _stream(stream)), "wl_eval")
+        if wilson_events is None:
+            _check(_lib.wl_eval(*args, _stream(stream)), "wl_eval")
+        else:
+            e0, e1 = (_event_handle(ev, stream) for ev in wilson_events)
+            _check(_lib.wl_eval_instrumented(*args, _stream(stream), e0, e1), "wl_eval_instrumented")
     return W_mean, group_sums
 
 

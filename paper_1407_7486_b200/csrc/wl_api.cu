@@ -77,6 +77,18 @@ wl_status wl_eval(const wl_field* field, const void* d_loops, wl_dtype loop_dtyp
                   int n_groups, wl_dtype compute, double* d_W_mean, double* d_group_sums,
                   void* d_workspace, size_t workspace_bytes, void* stream)
 {
+    return wl_eval_instrumented(field, d_loops, loop_dtype, n_loops, n_ppl, d_T, n_T, d_rho_cm, d_phi_cm, n_rho,
+                                n_groups, compute, d_W_mean, d_group_sums, d_workspace, workspace_bytes, stream,
+                                nullptr, nullptr);
+}
+
+wl_status wl_eval_instrumented(const wl_field* field, const void* d_loops, wl_dtype loop_dtype, int64_t n_loops,
+                               int n_ppl, const double* d_T, int n_T, const double* d_rho_cm,
+                               const double* d_phi_cm, int n_rho, int n_groups, wl_dtype compute,
+                               double* d_W_mean, double* d_group_sums, void* d_workspace,
+                               size_t workspace_bytes, void* stream, void* event_wilson_begin,
+                               void* event_wilson_end)
+{
     if (!field || !d_loops || !d_T || !d_rho_cm || !d_W_mean || !d_group_sums) return WL_ERR_INVALID_ARG;
     if (!dtype_ok(loop_dtype) || !dtype_ok(compute)) return WL_ERR_INVALID_ARG;
     if (!sizes_ok(n_loops, n_ppl, n_T, n_rho, n_groups)) return WL_ERR_INVALID_ARG;
@@ -91,8 +103,10 @@ wl_status wl_eval(const wl_field* field, const void* d_loops, wl_dtype loop_dtyp
     a.partial = reinterpret_cast<double*>(d_workspace);
     a.phase_out = nullptr; a.spin_out = nullptr;
     cudaStream_t s = (cudaStream_t)stream;
+    if (event_wilson_begin && cudaEventRecord((cudaEvent_t)event_wilson_begin, s) != cudaSuccess) return WL_ERR_CUDA;
     cudaError_t e = launch_wilson(plan, a, field->profile, compute, s);
     if (e != cudaSuccess) return e == cudaErrorInvalidValue ? WL_ERR_UNSUPPORTED : WL_ERR_CUDA;
+    if (event_wilson_end && cudaEventRecord((cudaEvent_t)event_wilson_end, s) != cudaSuccess) return WL_ERR_CUDA;
     e = launch_group_reduce(a.partial, plan.n_units, plan.units_per_group, n_groups, plan.n_grid, n_loops,
                             d_group_sums, d_W_mean, s);
     return e == cudaSuccess ? WL_OK : WL_ERR_CUDA;
