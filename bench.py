@@ -260,3 +260,117 @@ def run_ours(args, cfg):
     result_checksum = float(mean.sum().item())
     if not np.isfinite(result_checksum):
         raise SystemExit("bench.py: non-finite <W>")
+
+    # ---- e2e: the C-ABI call on HOST buffers (wl_eval_host), copies inside the timed region ----
+    e2e = None
+    if not args.no_e2e:
+        host_loops = torch.empty(loops.shape, dtype=loops.dtype, pin_memory=True)
+        host_loops.copy_(loops)
+        torch.cuda.synchronize()
+        hl = host_loops.numpy()
+        G_e2e = sh.n_groups
+        for _ in range(min(args.warmup, 2)):
+            api.wl_eval_host(field, hl, T, rho, phi, n_groups=G_e2e, compute=compute)
+        fence()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            hm, he, hg = api.wl_eval_host(field, hl, T, rho, phi, n_groups=G_e2e, compute=compute)
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        h2d = hl.nbytes + T.nbytes + rho.nbytes + (phi.nbytes if phi is not None else 0)
+        d2h = hm.nbytes + he.nbytes + hg.nbytes
+        e2e = {"value": evals_per_gpu * world * args.steps / dt, "unit": UNIT,
+               "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+               "ms_per_step": 1e3 * dt / args.steps,
+               "call": "wl_eval_host (per rank: its own loops; pinned host memory; wall clock, max over ranks)"}
+        if not np.array_equal(hm, W_mean.cpu().numpy()):
+            raise SystemExit("bench.py: wl_eval_host and wl_eval disagree")
+        del host_loops
+
+    if rank != 0:
+        if world > 1:
+            dist.barrier()
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of the dominant kernel (k_wilson), DESIGN.md section 5 ----
+    sm_max_mhz = clocks.get("sm_max_mhz") or 1965
+    k_ms = sum(wilson_ms) / len(wilson_ms)
+    if compute == "f32":
+        ops = (ALG_PLAIN_OPS + ALG_SFU_OPS) if cfg.profile == 1 else ALG_OPS_UNIFORM
+        peak = SM_COUNT * ISSUE_LANES_PER_CLK_SM * sm_max_mhz * 1e6
+        peak_how = ("derived: 148 SMs x 4 sub-partitions x 32 lanes x %d MHz (FP32 non-tensor issue roofline; "
+                    "FFMA micro-benchmark measured 123/128 of it, profiles/r01_pipe_rates.md)" % sm_max_mhz)
+        ops_how = "%d algorithmic FP32 lane-ops per point-eval (29 plain + 7 special-function, SURVEY.md 8(d))" % ops
+    else:
+        ops = 200 if cfg.profile == 1 else ALG_OPS_UNIFORM
+        peak = SM_COUNT * FP64_LANES_PER_CLK_SM * sm_max_mhz * 1e6
+        peak_how = "derived: 148 SMs x 64 FP64 lanes x %d MHz (DFMA micro-benchmark measured 63.8/64)" % sm_max_mhz
+        ops_how = "%d FP64 lane-ops per point-eval (DESIGN.md section 5)" % ops
+    achieved = ops * evals_per_gpu / (k_ms * 1e-3)
+    roofline = {
+        "bound": "alu", "kernel": "k_wilson", "achieved": achieved / 1e12, "peak": peak / 1e12,
+        "unit": "Tlane-op/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, compute)),
+        "kernel_ms": k_ms, "kernel_share_of_step": k_ms / ms_per_step,
+        "algorithmic_ops": ops_how, "peak_source": peak_how,
+        "sfu_frac": (ALG_SFU_OPS * evals_per_gpu / (k_ms * 1e-3)) / (SM_COUNT * SFU_LANES_PER_CLK_SM * sm_max_mhz * 1e6)
+        if (compute == "f32" and cfg.profile == 1) else None,
+        "hbm_GBps_algorithmic": loops.numel() * loops.element_size() / (k_ms * 1e-3) / 1e9,
+    }
+
+    # ---- cpu_baseline: the oracle as it stands, bounded sample, this box's host cores ----
+    cpu_baseline = None
+    if not args.no_cpu_baseline:
+        cores = affinity_cores()
+        n = oracle_sample_loops(cfg, cores, 256)
+        sample_loops = loops[:n].cpu().numpy()
+        rate, dt, threads = time_oracle(cfg, sample_loops, T, rho, phi)
+        cpu_baseline = {"value": rate, "unit": UNIT, "cores": threads, "kind": "oracle",
+                        "sample": "first %d whole loops x full %dx%d grid (%.1f s)" % (n, cfg.n_T, cfg.n_rho, dt)}
+
+    launches_per_step = api.wl_eval_launch_count(sh.n_loops, cfg.n_ppl, cfg.n_T, cfg.n_rho, sh.n_groups, compute) + 1
+    line = base_line(args, cfg, world)
+    line.update({
+        "value": value, "ms_per_step": ms_per_step, "dtype": compute,
+        "config": workload_config(cfg, world, compute),
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
+        "roofline": roofline, "cpu_baseline": cpu_baseline,
+        "checksum_sum_W_mean": result_checksum,
+    })
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_wilson launch from the `ncu --set full` capture
+# summarised under profiles/ (per launch, like `achieved`); None until measured for that workload.
+NCU_TRAFFIC_BYTES = {}
+
+
+def main():
+    ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
+    ap.add_argument("--workload", type=int, default=3, help="BASELINE.json config number (1-5); 3 = paper scale")
+    ap.add_argument("--compute", choices=("f32", "f64"), default=None)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.steps < 1 or args.warmup < 0:
+        raise SystemExit("--steps >= 1, --warmup >= 0")
+    from paper_1407_7486_b200 import inputs
+    cfg = inputs.config(args.workload)
+    if args.impl == "reference":
+        return run_reference(args, cfg)
+    return run_ours(args, cfg)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -241,6 +241,11 @@ static cudaError_t launch_r(const EvalPlan& plan, const EvalArgs& a, int profile
 
 cudaError_t launch_wilson(const EvalPlan& plan, const EvalArgs& a, int profile, wl_dtype compute, cudaStream_t s)
 {
+    if (compute == WL_F32 && profile == WL_PROFILE_SECH2 && a.phi == nullptr) {
+        EvalPlan p2 = plan;                              // grid points go in register pairs there
+        if (p2.P < 2) { p2.P = 2; p2.n_tiles = (p2.n_grid + kThreads * 2 - 1) / (kThreads * 2); }
+        return launch_wilson_sech2_f32(p2, a, s);
+    }
     return compute == WL_F32 ? launch_r<float>(plan, a, profile, s) : launch_r<double>(plan, a, profile, s);
 }
 
