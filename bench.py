@@ -43,7 +43,8 @@ ALG_OPS_UNIFORM = 4
 SM_COUNT = 148
 ISSUE_LANES_PER_CLK_SM = 128      # 4 sub-partitions x 1 warp instruction (32 lanes) per clock
 FP64_LANES_PER_CLK_SM = 64        # measured 63.8 (profiles/r01_pipe_rates.md)
-SFU_LANES_PER_CLK_SM = 16         # measured 15.96
+SFU_LANES_PER_CLK_SM = 16         # measured 15.9
+KERNEL_SFU_OPS = 5                # MUFU per point-eval in k_wilson_sech2_f32 (sqrt, rsqrt, 2 x ex2, rcp)
 
 
 def affinity_cores():
@@ -316,8 +317,9 @@ def run_ours(args, cfg):
         "unit": "Tlane-op/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, compute)),
         "kernel_ms": k_ms, "kernel_share_of_step": k_ms / ms_per_step,
         "algorithmic_ops": ops_how, "peak_source": peak_how,
-        "sfu_frac": (ALG_SFU_OPS * evals_per_gpu / (k_ms * 1e-3)) / (SM_COUNT * SFU_LANES_PER_CLK_SM * sm_max_mhz * 1e6)
-        if (compute == "f32" and cfg.profile == 1) else None,
+        # the special-function ops the kernel really issues (5 per point-eval) against the measured XU rate
+        "xu_pipe_frac": (KERNEL_SFU_OPS * evals_per_gpu / (k_ms * 1e-3)) / (SM_COUNT * SFU_LANES_PER_CLK_SM * sm_max_mhz * 1e6)
+        if (compute == "f32" and cfg.profile == 1 and phi is None) else None,
         "hbm_GBps_algorithmic": loops.numel() * loops.element_size() / (k_ms * 1e-3) / 1e9,
     }
 
@@ -349,7 +351,10 @@ def run_ours(args, cfg):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_wilson launch from the `ncu --set full` capture
 # summarised under profiles/ (per launch, like `achieved`); None until measured for that workload.
-NCU_TRAFFIC_BYTES = {}
+NCU_TRAFFIC_BYTES = {
+    # profiles/r01_wilson_f32_ncu.md: 279.2 MB read (the 268.4 MB ensemble once) + 58.8 MB written (partials)
+    ("cfg3_paper_scale", "f32"): 279201280 + 58751232,
+}
 
 
 def main():
