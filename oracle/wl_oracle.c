@@ -24,6 +24,10 @@
  * plus the unit-loop generator (d-loops, steps (1)-(5), eq. (10)-(11),
  * PAPER.md:65-81) driven by Philox4x32-10 (reading A11).
  *
+ * Also: the paper's own flux-tube profile f_lambda = rho^2/(lambda^2+rho^2)
+ * (eq. (68)) and the scalar-QED output W = cos(phase), pinned
+ * in tests/test_oracle_fluxtube_scalar.py.
+ *
  * Pins (tests/test_oracle_*.py, all -m "not gpu"): zero field, uniform-field
  * shoelace area, finite-N uniform closed form, Stokes flux of the sech^2
  * profile by independent quadrature, mpmath evaluation of the profile,
@@ -44,6 +48,7 @@
 
 #define WLO_PROFILE_UNIFORM 0
 #define WLO_PROFILE_SECH2 1
+#define WLO_PROFILE_FLUXTUBE 2   /* f_lambda(rho^2) = rho^2/(lambda^2+rho^2), eq. (68) */
 
 /* ------------------------------------------------------------------------- */
 /* Field profiles.  e is folded into the field strength: only eB, eB0 enter.  */
@@ -78,6 +83,10 @@ double wlo_field_g(int profile, const double *params, double rho)
 {
     if (profile == WLO_PROFILE_UNIFORM)
         return 0.5 * params[0];                 /* A = (B/2)(-y, x) */
+    if (profile == WLO_PROFILE_FLUXTUBE)
+        /* eq. (14) with eq. (68): e A_phi/rho = (eF/2pi) f_lambda/rho^2 = script-F/(lambda^2+rho^2),
+         * params = {script-F (eq. (17)), lambda} */
+        return params[0] / (params[1] * params[1] + rho * rho);
     return params[0] * sech2_h(rho / params[1]);
 }
 
@@ -86,6 +95,12 @@ double wlo_field_b(int profile, const double *params, double rho)
 {
     if (profile == WLO_PROFILE_UNIFORM)
         return params[0];
+    if (profile == WLO_PROFILE_FLUXTUBE) {
+        /* eq. (15) with eq. (68): e B_z = (eF/2pi rho) d f_lambda/d rho = 2 script-F lambda^2/(lambda^2+rho^2)^2 */
+        double l2 = params[1] * params[1];
+        double D = l2 + rho * rho;
+        return 2.0 * params[0] * l2 / (D * D);
+    }
     return params[0] * sech2_b(rho / params[1]);
 }
 
@@ -119,7 +134,29 @@ void wlo_loop_phase_spin(int profile, const double *params,
 /*   W_loop, phase_loop, spin_loop: nullable, [n_loops][n_T][n_rho]           */
 /* Returns 0, or -1 on a bad argument.                                        */
 /* ------------------------------------------------------------------------- */
+/* scalar != 0: scalar QED, W = cos(phase) only (the paper's Wsscal;         */
+/* exact uniform-field average eq. (43)); scalar == 0: fermion, eq. (18).               */
+int wlo_eval_particle(int profile, const double *params, int scalar,
+             const double *loops, int64_t n_loops, int N,
+             const double *T, int n_T,
+             const double *rho_cm, const double *phi_cm, int n_rho,
+             int n_groups,
+             double *W_mean, double *group_sums,
+             double *W_loop, double *phase_loop, double *spin_loop);
+
 int wlo_eval(int profile, const double *params,
+             const double *loops, int64_t n_loops, int N,
+             const double *T, int n_T,
+             const double *rho_cm, const double *phi_cm, int n_rho,
+             int n_groups,
+             double *W_mean, double *group_sums,
+             double *W_loop, double *phase_loop, double *spin_loop)
+{
+    return wlo_eval_particle(profile, params, 0, loops, n_loops, N, T, n_T, rho_cm, phi_cm, n_rho, n_groups,
+                             W_mean, group_sums, W_loop, phase_loop, spin_loop);
+}
+
+int wlo_eval_particle(int profile, const double *params, int scalar,
              const double *loops, int64_t n_loops, int N,
              const double *T, int n_T,
              const double *rho_cm, const double *phi_cm, int n_rho,
@@ -145,7 +182,7 @@ int wlo_eval(int profile, const double *params,
                 double phase, spin;
                 wlo_loop_phase_spin(profile, params, y, N, T[t], cx, cy, &phase, &spin);
                 int64_t o = l * n_grid + (int64_t)t * n_rho + r;
-                W[o] = cos(phase) * cosh(spin);
+                W[o] = scalar ? cos(phase) : cos(phase) * cosh(spin);
                 if (phase_loop) phase_loop[o] = phase;
                 if (spin_loop) spin_loop[o] = spin;
             }

@@ -15,6 +15,7 @@ from . import build as _build
 
 UNIFORM = 0
 SECH2 = 1
+FLUXTUBE = 2
 
 _lib = None
 _dp = C.POINTER(C.c_double)
@@ -34,6 +35,9 @@ def lib():
         L.wlo_eval.restype = C.c_int
         L.wlo_eval.argtypes = [C.c_int, _dp, _dp, C.c_int64, C.c_int, _dp, C.c_int, _dp, _dp,
                                C.c_int, C.c_int, _dp, _dp, _dp, _dp, _dp]
+        L.wlo_eval_particle.restype = C.c_int
+        L.wlo_eval_particle.argtypes = [C.c_int, _dp, C.c_int, _dp, C.c_int64, C.c_int, _dp, C.c_int, _dp, _dp,
+                                        C.c_int, C.c_int, _dp, _dp, _dp, _dp, _dp]
         L.wlo_finalize.restype = C.c_int
         L.wlo_finalize.argtypes = [_dp, C.c_int, C.c_int64, C.c_int64, _dp, _dp, _dp]
         L.wlo_philox4x32_10.restype = None
@@ -80,8 +84,8 @@ def loop_phase_spin(profile, params, y, T, cx, cy):
     return ph.value, sp.value
 
 
-def evaluate(profile, params, loops, T, rho_cm, phi_cm=None, n_groups=1, per_loop=False):
-    """Whole-ensemble evaluation.
+def evaluate(profile, params, loops, T, rho_cm, phi_cm=None, n_groups=1, per_loop=False, scalar=False):
+    """Whole-ensemble evaluation (scalar=True: scalar QED, W = cos(phase), eq. (19)-(20), (43)).
 
     loops [n_loops][N][2] (float32 storage is promoted exactly to float64).
     Returns dict(W_mean [n_T][n_rho], group_sums [G][n_T][n_rho]) and, if per_loop,
@@ -102,8 +106,8 @@ def evaluate(profile, params, loops, T, rho_cm, phi_cm=None, n_groups=1, per_loo
     W = ph = sp = None
     if per_loop:
         W, ph, sp = (np.empty((nl, nT, nr)) for _ in range(3))
-    rc = lib().wlo_eval(profile, _p(pr), _p(y), nl, N, _p(T), nT, _p(rho), _p(phi), nr, n_groups,
-                        _p(mean), _p(gs), _p(W), _p(ph), _p(sp))
+    rc = lib().wlo_eval_particle(profile, _p(pr), 1 if scalar else 0, _p(y), nl, N, _p(T), nT, _p(rho), _p(phi),
+                                 nr, n_groups, _p(mean), _p(gs), _p(W), _p(ph), _p(sp))
     if rc != 0:
         raise ValueError("wlo_eval: invalid argument")
     out = {"W_mean": mean, "group_sums": gs}
