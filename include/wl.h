@@ -55,10 +55,20 @@ typedef enum {
  * (eq. (13)-(17)).  The charge e is folded into the strength. */
 typedef enum {
     WL_PROFILE_UNIFORM = 0,   /* params {eB}:           B_z = B, A = (B/2)(-y, x)            */
-    WL_PROFILE_SECH2 = 1      /* params {eB0, lambda}:  B_z = B0 sech^2(rho/lambda),
+    WL_PROFILE_SECH2 = 1,     /* params {eB0, lambda}:  B_z = B0 sech^2(rho/lambda),
                                  Phi = 2 pi B0 [lambda rho tanh(rho/lambda)
                                                - lambda^2 ln cosh(rho/lambda)]               */
+    WL_PROFILE_FLUXTUBE = 2   /* params {script-F, lambda}: the paper's validation profile
+                                 f_lambda = rho^2/(lambda^2+rho^2), eq. (68), in
+                                 A_phi = F f_lambda/(2 pi rho), eq. (14); script-F = eF/2pi, eq. (17):
+                                 e A_phi/rho = script-F/(lambda^2+rho^2),
+                                 e B_z = 2 script-F lambda^2/(lambda^2+rho^2)^2              */
 } wl_profile;
+
+/* What the loop belongs to (eq. (18)): a fermion loop carries the spin factor,
+ * W = cos(phase) cosh(spin); a scalar loop (scalar QED, the paper's Wsscal)
+ * has W = cos(phase) only (exact uniform-field average eq. (43)). */
+typedef enum { WL_FERMION = 0, WL_SCALAR = 1 } wl_particle;
 
 typedef enum { WL_F32 = 0, WL_F64 = 1 } wl_dtype;
 
@@ -69,6 +79,10 @@ typedef struct wl_field wl_field;   /* opaque, host memory, immutable after crea
  * a wrong n_params or an unknown profile give WL_ERR_INVALID_ARG and *out = NULL.
  * The caller releases it with wl_field_destroy.  Host-only; no CUDA call. */
 wl_status wl_field_create(wl_profile profile, const double* h_params, int n_params, wl_field** out);
+/* Same with the particle type stated (wl_field_create = WL_FERMION); FLUXTUBE: n_params == 2,
+ * {script-F, lambda}, lambda > 0.  An unknown particle gives WL_ERR_INVALID_ARG. */
+wl_status wl_field_create_particle(wl_profile profile, const double* h_params, int n_params,
+                                   wl_particle particle, wl_field** out);
 void wl_field_destroy(wl_field* field);   /* NULL is allowed */
 
 /* Seeded unit-loop ensemble: d-loops, steps (1)-(5), eq. (10)-(11), PAPER.md:65-81,
@@ -142,9 +156,10 @@ wl_status wl_jackknife_finalize(const double* d_group_sums, int n_groups, int64_
 
 /* End-to-end convenience call on HOST buffers: allocates device memory, copies
  * h_loops / grids to the device, runs wl_eval + wl_jackknife_finalize on an
- * internal stream, copies h_W_mean[n_T][n_rho], h_err[n_T][n_rho] and
- * h_group_sums[G][n_T][n_rho] back, frees the device memory and returns after
- * everything has completed.  h_phi_cm, h_err and h_group_sums may be NULL.
+ * internal stream (the copy of all but the first few jackknife groups overlaps the
+ * evaluation of those; same bits as one wl_eval), copies h_W_mean[n_T][n_rho], h_err[n_T][n_rho]
+ * and h_group_sums[G][n_T][n_rho] back, returns the device memory to the library's pool (see
+ * wl_eval_host_trim) and returns after everything has completed.  h_phi_cm, h_err and h_group_sums may be NULL.
  * This is the only call that allocates, copies and synchronises. */
 wl_status wl_eval_host(const wl_field* field,
                        const void* h_loops, wl_dtype loop_dtype, int64_t n_loops, int n_ppl,
@@ -152,6 +167,10 @@ wl_status wl_eval_host(const wl_field* field,
                        const double* h_rho_cm, const double* h_phi_cm, int n_rho,
                        int n_groups, wl_dtype compute,
                        double* h_W_mean, double* h_err, double* h_group_sums);
+
+/* wl_eval_host takes its device memory from a private stream-ordered pool that keeps it between
+ * calls; this returns the pool's unused memory to the device.  WL_OK if there is nothing to release. */
+wl_status wl_eval_host_trim(void);
 
 /* Number of kernels wl_eval enqueues for these sizes (for launch accounting). */
 int wl_eval_launch_count(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups,

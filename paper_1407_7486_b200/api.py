@@ -17,6 +17,9 @@ LIB_PATH = os.path.join(HERE, "libwl.so")
 WL_OK = 0
 PROFILE_UNIFORM = 0
 PROFILE_SECH2 = 1
+PROFILE_FLUXTUBE = 2
+FERMION = 0
+SCALAR = 1
 F32 = 0
 F64 = 1
 
@@ -28,6 +31,8 @@ _lib = C.CDLL(LIB_PATH)
 _vp, _dp, _i64, _int, _u64, _sz = C.c_void_p, C.c_void_p, C.c_int64, C.c_int, C.c_uint64, C.c_size_t
 _lib.wl_field_create.restype = _int
 _lib.wl_field_create.argtypes = [_int, C.POINTER(C.c_double), _int, C.POINTER(_vp)]
+_lib.wl_field_create_particle.restype = _int
+_lib.wl_field_create_particle.argtypes = [_int, C.POINTER(C.c_double), _int, _int, C.POINTER(_vp)]
 _lib.wl_field_destroy.restype = None
 _lib.wl_field_destroy.argtypes = [_vp]
 _lib.wl_loops_generate.restype = _int
@@ -49,6 +54,8 @@ _lib.wl_jackknife_finalize.argtypes = [_dp, _int, _i64, _int, _int, _dp, _dp, _d
 _lib.wl_eval_host.restype = _int
 _lib.wl_eval_host.argtypes = [_vp, _vp, _int, _i64, _int, _dp, _int, _dp, _dp, _int, _int, _int, _dp, _dp,
                               _dp]
+_lib.wl_eval_host_trim.restype = _int
+_lib.wl_eval_host_trim.argtypes = []
 _lib.wl_status_string.restype = C.c_char_p
 _lib.wl_status_string.argtypes = [_int]
 _lib.wl_version.restype = C.c_char_p
@@ -108,13 +115,15 @@ def _ptr(t):
 class Field:
     """Owns a wl_field* (wl_field_create / wl_field_destroy)."""
 
-    def __init__(self, profile, params):
+    def __init__(self, profile, params, particle=FERMION):
         arr = (C.c_double * len(params))(*[float(p) for p in params])
         h = C.c_void_p()
-        _check(_lib.wl_field_create(int(profile), arr, len(params), C.byref(h)), "wl_field_create")
+        _check(_lib.wl_field_create_particle(int(profile), arr, len(params), int(particle), C.byref(h)),
+               "wl_field_create_particle")
         self._h = h
         self.profile = int(profile)
         self.params = tuple(float(p) for p in params)
+        self.particle = int(particle)
 
     def __del__(self, _destroy=_lib.wl_field_destroy):
         h, self._h = getattr(self, "_h", None), None
@@ -124,6 +133,11 @@ class Field:
 
 def wl_field_create(profile, params) -> Field:
     return Field(profile, params)
+
+
+def wl_field_create_particle(profile, params, particle) -> Field:
+    """particle = FERMION (W = cos(phase) cosh(spin)) or SCALAR (W = cos(phase))."""
+    return Field(profile, params, particle)
 
 
 def wl_loops_generate(n_loops, n_ppl, seed, dtype=torch.float64, loop_begin=0, out=None, device="cuda",
@@ -257,3 +271,8 @@ def wl_eval_host(field, loops, T, rho_cm, phi_cm=None, n_groups=2, compute=torch
                              p(rho), p(phi), n_rho, int(n_groups), _dtype_code(compute), p(mean), p(err),
                              p(gs)), "wl_eval_host")
     return mean, err, gs
+
+
+def wl_eval_host_trim():
+    """Returns the unused memory of wl_eval_host's private pool to the device."""
+    _check(_lib.wl_eval_host_trim(), "wl_eval_host_trim")

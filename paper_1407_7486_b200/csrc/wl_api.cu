@@ -25,22 +25,30 @@ extern "C" {
 
 wl_status wl_field_create(wl_profile profile, const double* h_params, int n_params, wl_field** out)
 {
+    return wl_field_create_particle(profile, h_params, n_params, WL_FERMION, out);
+}
+
+wl_status wl_field_create_particle(wl_profile profile, const double* h_params, int n_params,
+                                   wl_particle particle, wl_field** out)
+{
     if (!out) return WL_ERR_INVALID_ARG;
     *out = nullptr;
     if (!h_params) return WL_ERR_INVALID_ARG;
     if (profile == WL_PROFILE_UNIFORM) {
         if (n_params != 1 || !std::isfinite(h_params[0])) return WL_ERR_INVALID_ARG;
-    } else if (profile == WL_PROFILE_SECH2) {
+    } else if (profile == WL_PROFILE_SECH2 || profile == WL_PROFILE_FLUXTUBE) {
         if (n_params != 2 || !std::isfinite(h_params[0]) || !std::isfinite(h_params[1]) || !(h_params[1] > 0.0))
             return WL_ERR_INVALID_ARG;
     } else {
         return WL_ERR_INVALID_ARG;
     }
+    if (particle != WL_FERMION && particle != WL_SCALAR) return WL_ERR_INVALID_ARG;
     wl_field* f = new (std::nothrow) wl_field;
     if (!f) return WL_ERR_INVALID_ARG;
     f->profile = (int)profile;
     f->p0 = h_params[0];
     f->p1 = (n_params > 1) ? h_params[1] : 0.0;
+    f->scalar = (particle == WL_SCALAR);
     *out = f;
     return WL_OK;
 }
@@ -99,7 +107,7 @@ wl_status wl_eval_instrumented(const wl_field* field, const void* d_loops, wl_dt
     EvalArgs a;
     a.loops = d_loops; a.loops_are_f64 = (loop_dtype == WL_F64); a.n_loops = n_loops; a.n_ppl = n_ppl;
     a.T = d_T; a.rho = d_rho_cm; a.phi = d_phi_cm; a.n_T = n_T; a.n_rho = n_rho;
-    a.p0 = field->p0; a.p1 = field->p1;
+    a.p0 = field->p0; a.p1 = field->p1; a.scalar = field->scalar;
     a.partial = reinterpret_cast<double*>(d_workspace);
     a.phase_out = nullptr; a.spin_out = nullptr;
     cudaStream_t s = (cudaStream_t)stream;
@@ -124,7 +132,7 @@ wl_status wl_eval_per_loop(const wl_field* field, const void* d_loops, wl_dtype 
     EvalArgs a;
     a.loops = d_loops; a.loops_are_f64 = (loop_dtype == WL_F64); a.n_loops = n_loops; a.n_ppl = n_ppl;
     a.T = d_T; a.rho = d_rho_cm; a.phi = d_phi_cm; a.n_T = n_T; a.n_rho = n_rho;
-    a.p0 = field->p0; a.p1 = field->p1;
+    a.p0 = field->p0; a.p1 = field->p1; a.scalar = field->scalar;
     a.partial = d_W; a.phase_out = d_phase; a.spin_out = d_spin;
     cudaError_t e = launch_wilson(plan, a, field->profile, compute, (cudaStream_t)stream);
     if (e != cudaSuccess) return e == cudaErrorInvalidValue ? WL_ERR_UNSUPPORTED : WL_ERR_CUDA;

@@ -140,7 +140,7 @@ k_wilson(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit, int chunk_poin
             const double T = a.T[g / a.n_rho];
             const double phase = prof.g_scale() * dph[j];
             const double spin = prof.b_scale() * (T / double(N)) * dsp[j];
-            const double W = cos(phase) * cosh(spin);
+            const double W = a.scalar ? cos(phase) : cos(phase) * cosh(spin);
             Wsum[j] += W;
             if (gp[j] < n_grid) {
                 if (a.phase_out) a.phase_out[loop * n_grid + gp[j]] = phase;
@@ -236,6 +236,8 @@ static cudaError_t launch_r(const EvalPlan& plan, const EvalArgs& a, int profile
         return phi ? launch_p<Real, Uniform, true>(plan, a, s) : launch_p<Real, Uniform, false>(plan, a, s);
     if (profile == WL_PROFILE_SECH2)
         return phi ? launch_p<Real, Sech2, true>(plan, a, s) : launch_p<Real, Sech2, false>(plan, a, s);
+    if (profile == WL_PROFILE_FLUXTUBE)
+        return phi ? launch_p<Real, FluxTube, true>(plan, a, s) : launch_p<Real, FluxTube, false>(plan, a, s);
     return cudaErrorInvalidValue;
 }
 

@@ -29,6 +29,7 @@ __device__ __forceinline__ float mufu_rcp(float x)   { float y; asm("rcp.approx.
 
 template <typename Real> struct Uniform;
 template <typename Real> struct Sech2;
+template <typename Real> struct FluxTube;
 
 // ---------------------------------------------------------------- uniform field
 // g = eB/2, b = eB: the terms are the bare cross product and 1.
@@ -120,6 +121,34 @@ struct Sech2<double> {
     }
     __device__ double b_scale() const { return 4.0 * eB0; }
     __device__ double g_scale() const { return eB0; }
+};
+
+// ---------------------------------------------------------------- flux tube, eq. (68)
+// f_lambda = rho^2/(lambda^2+rho^2):  g = script-F/(lambda^2+rho^2),  b = 2 script-F lambda^2/(lambda^2+rho^2)^2
+// (eq. (14), (15), (17)).  With a = 1 + w/lambda^2:  g = (script-F/lambda^2)/a_m,
+// b = (2 script-F/lambda^2)/a_p^2.  No square root: the profile is a function of rho^2.
+template <typename Real>
+struct FluxTube {
+    static constexpr bool kNeedsRadius = true;
+    double F, lambda;
+    Real il2;
+    __device__ explicit FluxTube(double p0, double p1) : F(p0), lambda(p1), il2(Real(1.0 / (p1 * p1))) {}
+    __device__ __forceinline__ void terms(float wp, float wm, float& bt, float& gt) const
+    {
+        const float ap = fmaf(wp, il2, 1.0f), am = fmaf(wm, il2, 1.0f);
+        const float r = mufu_rcp(ap * am);                   // one reciprocal for point and midpoint
+        const float ip = r * am;
+        gt = r * ap;
+        bt = ip * ip;
+    }
+    __device__ __forceinline__ void terms(double wp, double wm, double& bt, double& gt) const
+    {
+        const double ip = 1.0 / fma(wp, (double)il2, 1.0);
+        gt = 1.0 / fma(wm, (double)il2, 1.0);
+        bt = ip * ip;
+    }
+    __device__ double b_scale() const { return 2.0 * F / (lambda * lambda); }
+    __device__ double g_scale() const { return F / (lambda * lambda); }
 };
 
 }  // namespace wl

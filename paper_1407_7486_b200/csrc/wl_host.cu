@@ -4,17 +4,62 @@
 
 namespace {
 
+// Device memory of wl_eval_host comes from a private stream-ordered pool (one per device) that keeps
+// what it has been given between calls (release threshold = max), so that a second call of the
+// same size pays no cudaMalloc/cudaFree; wl_eval_host_trim() gives the memory back.
+cudaMemPool_t g_pool[64] = {};
+
+cudaError_t host_pool(cudaMemPool_t* out)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    if (!g_pool[dev]) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t pool;
+        e = cudaMemPoolCreate(&pool, &props);
+        if (e != cudaSuccess) return e;
+        unsigned long long keep = ~0ull;
+        e = cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        if (e != cudaSuccess) { cudaMemPoolDestroy(pool); return e; }
+        g_pool[dev] = pool;
+    }
+    *out = g_pool[dev];
+    return cudaSuccess;
+}
+
 struct DeviceBuffers {
     void* p[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
-    cudaStream_t s = nullptr;
+    cudaStream_t s = nullptr, copy = nullptr;
+    cudaEvent_t ev[2] = {nullptr, nullptr};
     ~DeviceBuffers()
     {
-        for (void* q : p) if (q) cudaFree(q);
+        if (s) {
+            for (void* q : p) if (q) cudaFreeAsync(q, s);
+            cudaStreamSynchronize(s);
+        }
+        for (cudaEvent_t e : ev) if (e) cudaEventDestroy(e);
         if (s) cudaStreamDestroy(s);
+        if (copy) cudaStreamDestroy(copy);
     }
 };
 
 }  // namespace
+
+extern "C" wl_status wl_eval_host_trim(void)
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return WL_ERR_CUDA; }
+    if (dev >= 0 && dev < 64 && g_pool[dev]) {
+        if (cudaMemPoolTrimTo(g_pool[dev], 0) != cudaSuccess) { cudaGetLastError(); return WL_ERR_CUDA; }
+    }
+    return WL_OK;
+}
 
 extern "C" wl_status wl_eval_host(const wl_field* field, const void* h_loops, wl_dtype loop_dtype,
                                   int64_t n_loops, int n_ppl, const double* h_T, int n_T,
@@ -33,26 +78,66 @@ extern "C" wl_status wl_eval_host(const wl_field* field, const void* h_loops, wl
     enum { LOOPS, T, RHO, PHI, MEAN, GS, ERR, WS };
 #define WL_TRY(call) do { if ((call) != cudaSuccess) { cudaGetLastError(); return WL_ERR_CUDA; } } while (0)
     WL_TRY(cudaStreamCreateWithFlags(&d.s, cudaStreamNonBlocking));
-    WL_TRY(cudaMalloc(&d.p[LOOPS], loop_bytes));
-    WL_TRY(cudaMalloc(&d.p[T], n_T * sizeof(double)));
-    WL_TRY(cudaMalloc(&d.p[RHO], n_rho * sizeof(double)));
-    if (h_phi_cm) WL_TRY(cudaMalloc(&d.p[PHI], n_rho * sizeof(double)));
-    WL_TRY(cudaMalloc(&d.p[MEAN], 2 * n_grid * sizeof(double)));          // W_mean, then finalised mean
-    WL_TRY(cudaMalloc(&d.p[GS], (size_t)n_groups * n_grid * sizeof(double)));
-    WL_TRY(cudaMalloc(&d.p[ERR], n_grid * sizeof(double)));
-    WL_TRY(cudaMalloc(&d.p[WS], ws));
+    WL_TRY(cudaStreamCreateWithFlags(&d.copy, cudaStreamNonBlocking));
+    for (cudaEvent_t& e : d.ev) WL_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    cudaMemPool_t pool;
+    WL_TRY(host_pool(&pool));
+#define WL_ALLOC(slot, bytes) WL_TRY(cudaMallocFromPoolAsync(&d.p[slot], (bytes), pool, d.s))
+    WL_ALLOC(LOOPS, loop_bytes);
+    WL_ALLOC(T, n_T * sizeof(double));
+    WL_ALLOC(RHO, n_rho * sizeof(double));
+    if (h_phi_cm) WL_ALLOC(PHI, n_rho * sizeof(double));
+    WL_ALLOC(MEAN, 2 * n_grid * sizeof(double));          // W_mean, then finalised mean
+    WL_ALLOC(GS, (size_t)n_groups * n_grid * sizeof(double));
+    WL_ALLOC(ERR, n_grid * sizeof(double));
+    WL_ALLOC(WS, ws);
+#undef WL_ALLOC
 
-    WL_TRY(cudaMemcpyAsync(d.p[LOOPS], h_loops, loop_bytes, cudaMemcpyHostToDevice, d.s));
     WL_TRY(cudaMemcpyAsync(d.p[T], h_T, n_T * sizeof(double), cudaMemcpyHostToDevice, d.s));
     WL_TRY(cudaMemcpyAsync(d.p[RHO], h_rho_cm, n_rho * sizeof(double), cudaMemcpyHostToDevice, d.s));
     if (h_phi_cm) WL_TRY(cudaMemcpyAsync(d.p[PHI], h_phi_cm, n_rho * sizeof(double), cudaMemcpyHostToDevice, d.s));
 
+    // Pipeline over chunks of whole jackknife groups: the copy of chunk 1 (copy stream) overlaps
+    // k_wilson on chunk 0 (compute stream).  The units, their order and the partial-sum layout are
+    // exactly those of one wl_eval over the whole ensemble, so the result has the same bits.
+    const wl::EvalPlan plan = wl::make_eval_plan(n_loops, n_ppl, n_T, n_rho, n_groups, compute, false);
+    const int64_t per_group = n_loops / n_groups;
+    // Two chunks: a small first one (1/32 of the groups) whose evaluation hides the copy of the rest
+    // (H2D moves a group ~30x faster than k_wilson evaluates it); more chunks would only add launch tails.
+    const int n_chunks = n_groups >= 2 ? 2 : 1;
+    const int g_first = n_groups >= 2 ? (n_groups / 32 > 0 ? n_groups / 32 : 1) : n_groups;
+    const size_t loop_stride = (size_t)n_ppl * 2 * (loop_dtype == WL_F64 ? 8 : 4);
     double* mean = reinterpret_cast<double*>(d.p[MEAN]);
-    wl_status st = wl_eval(field, d.p[LOOPS], loop_dtype, n_loops, n_ppl,
-                           reinterpret_cast<const double*>(d.p[T]), n_T,
-                           reinterpret_cast<const double*>(d.p[RHO]), reinterpret_cast<const double*>(d.p[PHI]),
-                           n_rho, n_groups, compute, mean, reinterpret_cast<double*>(d.p[GS]), d.p[WS], ws, d.s);
-    if (st != WL_OK) return st;
+    double* partial = reinterpret_cast<double*>(d.p[WS]);
+    WL_TRY(cudaEventRecord(d.ev[1], d.s));                    // the loop buffer exists (stream-ordered allocation)
+    WL_TRY(cudaStreamWaitEvent(d.copy, d.ev[1], 0));
+    for (int c = 0; c < n_chunks; ++c) {
+        const int g0 = (c == 0) ? 0 : g_first, g1 = (c == n_chunks - 1) ? n_groups : g_first;
+        const int64_t l0 = g0 * per_group, nl = (g1 - g0) * per_group;
+        if (nl == 0) continue;
+        char* dst = reinterpret_cast<char*>(d.p[LOOPS]) + (size_t)l0 * loop_stride;
+        WL_TRY(cudaMemcpyAsync(dst, reinterpret_cast<const char*>(h_loops) + (size_t)l0 * loop_stride,
+                               (size_t)nl * loop_stride, cudaMemcpyHostToDevice, d.copy));
+        WL_TRY(cudaEventRecord(d.ev[0], d.copy));
+        WL_TRY(cudaStreamWaitEvent(d.s, d.ev[0], 0));
+        wl::EvalPlan sub = plan;
+        sub.n_units = nl / plan.loops_per_unit;
+        wl::EvalArgs a;
+        a.loops = dst; a.loops_are_f64 = (loop_dtype == WL_F64); a.n_loops = nl; a.n_ppl = n_ppl;
+        a.T = reinterpret_cast<const double*>(d.p[T]); a.rho = reinterpret_cast<const double*>(d.p[RHO]);
+        a.phi = reinterpret_cast<const double*>(d.p[PHI]); a.n_T = n_T; a.n_rho = n_rho;
+        a.p0 = field->p0; a.p1 = field->p1; a.scalar = field->scalar;
+        a.partial = partial + (size_t)(l0 / plan.loops_per_unit) * plan.n_grid;
+        a.phase_out = nullptr; a.spin_out = nullptr;
+        cudaError_t e = wl::launch_wilson(sub, a, field->profile, compute, d.s);
+        if (e != cudaSuccess) { cudaGetLastError(); return e == cudaErrorInvalidValue ? WL_ERR_UNSUPPORTED : WL_ERR_CUDA; }
+    }
+    if (wl::launch_group_reduce(partial, plan.n_units, plan.units_per_group, n_groups, plan.n_grid, n_loops,
+                                reinterpret_cast<double*>(d.p[GS]), mean, d.s) != cudaSuccess) {
+        cudaGetLastError();
+        return WL_ERR_CUDA;
+    }
+    wl_status st = WL_OK;
     if (h_err) {
         st = wl_jackknife_finalize(reinterpret_cast<const double*>(d.p[GS]), n_groups, n_loops, n_T, n_rho,
                                    mean + n_grid, reinterpret_cast<double*>(d.p[ERR]), nullptr, d.s);

@@ -10,7 +10,8 @@
 struct wl_field {
     int profile;        // wl_profile
     double p0;          // UNIFORM: eB      SECH2: eB0
-    double p1;          // UNIFORM: unused  SECH2: lambda
+    double p1;          // UNIFORM: unused  SECH2, FLUXTUBE: lambda   (p0 of FLUXTUBE: script-F)
+    int scalar;         // 1: W = cos(phase) (WL_SCALAR), 0: W = cos(phase) cosh(spin)
 };
 
 namespace wl {
@@ -42,6 +43,7 @@ struct EvalArgs {
     const double* phi;          // [n_rho] or null
     int n_T, n_rho;
     double p0, p1;              // field parameters
+    int scalar;                 // W = cos(phase) only
     double* partial;            // [n_units][n_grid]
     double* phase_out;          // per-loop mode only, nullable
     double* spin_out;           // per-loop mode only, nullable

@@ -223,7 +223,7 @@ k_wilson_sech2_f32(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit)
             const double T = a.T[g / a.n_rho];
             const double phase = g_scale * dph[j];
             const double spin = b_scale * (T / double(N)) * dsp[j];
-            const double W = cos(phase) * cosh(spin);
+            const double W = a.scalar ? cos(phase) : cos(phase) * cosh(spin);
             Wsum[j] += W;
             if (gp[j] < n_grid) {
                 if (a.phase_out) a.phase_out[loop * n_grid + gp[j]] = phase;

@@ -17,6 +17,7 @@ import numpy as np
 
 UNIFORM = 0
 SECH2 = 1
+FLUXTUBE = 2      # the paper's validation profile, eq. (68)
 
 
 @dataclass(frozen=True)

@@ -56,7 +56,15 @@ def test_field_create_validation(lib):
     st, h = create(1, [1.0, 0.5])
     assert st == 0 and h.value
     lib.wl_field_destroy(h)
-    for profile, params in ((0, [1.0, 2.0]), (1, [1.0]), (1, [1.0, 0.0]), (1, [1.0, -1.0]),
+    st, h = create(2, [10.0, 1.0])                                   # flux tube, eq. (68)
+    assert st == 0 and h.value
+    lib.wl_field_destroy(h)
+    lib.wl_field_create_particle.argtypes = [C.c_int, C.POINTER(C.c_double), C.c_int, C.c_int, C.POINTER(C.c_void_p)]
+    arr, h = (C.c_double * 2)(1.0, 1.0), C.c_void_p()
+    assert lib.wl_field_create_particle(1, arr, 2, 1, C.byref(h)) == 0 and h.value          # scalar loop
+    lib.wl_field_destroy(h)
+    assert lib.wl_field_create_particle(1, arr, 2, 2, C.byref(h)) == 1 and not h.value      # unknown particle
+    for profile, params in ((0, [1.0, 2.0]), (1, [1.0]), (1, [1.0, 0.0]), (1, [1.0, -1.0]), (2, [1.0]), (2, [1.0, 0.0]),
                             (1, [float("nan"), 1.0]), (0, [float("inf")]), (7, [1.0])):
         st, h = create(profile, params)
         assert st == 1 and not h.value

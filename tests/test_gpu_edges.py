@@ -186,6 +186,17 @@ def test_host_call_equals_device_call(api):
     hm, he, hg = api.wl_eval_host(f, loops.cpu().numpy(), T, rho, None, n_groups=16, compute="f32")
     assert np.array_equal(hm, mean.cpu().numpy()) and np.array_equal(hg, gs.cpu().numpy())
     assert np.array_equal(he, fe.cpu().numpy())
+    # a second call reuses the pooled device memory; G = 1 (no error bars, one chunk); FP64 loops with phi
+    hm2, _, hg2 = api.wl_eval_host(f, loops.cpu().numpy(), T, rho, None, n_groups=16, compute="f32")
+    assert np.array_equal(hm2, hm) and np.array_equal(hg2, hg)
+    y64 = loops.double().cpu().numpy()
+    phi = np.linspace(0.0, 3.0, len(rho))
+    m1, g1 = api.wl_eval(f, loops.double(), dev(T), dev(rho), dev(phi), n_groups=1, compute="f64")
+    torch.cuda.synchronize()
+    hm3, _, hg3 = api.wl_eval_host(f, y64, T, rho, phi, n_groups=2, compute="f64")
+    assert np.array_equal(hg3.sum(0), hg3[0] + hg3[1])
+    assert np.max(np.abs(hm3 - m1.cpu().numpy())) < 1e-13 * np.abs(hm3).max()
+    api.wl_eval_host_trim()
 
 
 def test_error_statuses(api):
