@@ -40,6 +40,7 @@ UNIT = "point-evals/s"
 ALG_PLAIN_OPS = 29
 ALG_SFU_OPS = 7
 ALG_OPS_UNIFORM = 4
+ALG_F64_OPS_SECH2 = 98            # FP64-pipe lane-ops per point-eval, branch-free formulation
 SM_COUNT = 148
 ISSUE_LANES_PER_CLK_SM = 128      # 4 sub-partitions x 1 warp instruction (32 lanes) per clock
 FP64_LANES_PER_CLK_SM = 64        # measured 63.8 (profiles/r01_pipe_rates.md)
@@ -307,7 +308,7 @@ def run_ours(args, cfg):
                     "FFMA micro-benchmark measured 123/128 of it, profiles/r01_pipe_rates.md)" % sm_max_mhz)
         ops_how = "%d algorithmic FP32 lane-ops per point-eval (29 plain + 7 special-function, SURVEY.md 8(d))" % ops
     else:
-        ops = 200 if cfg.profile == 1 else ALG_OPS_UNIFORM
+        ops = ALG_F64_OPS_SECH2 if cfg.profile == 1 else ALG_OPS_UNIFORM
         peak = SM_COUNT * FP64_LANES_PER_CLK_SM * sm_max_mhz * 1e6
         peak_how = "derived: 148 SMs x 64 FP64 lanes x %d MHz (DFMA micro-benchmark measured 63.8/64)" % sm_max_mhz
         ops_how = "%d FP64 lane-ops per point-eval (DESIGN.md section 5)" % ops

@@ -8,7 +8,8 @@ in w and reports the maximum relative error on a fine grid.
 
 Usage:  python gen_h_poly.py <w_max> <degree>          h(w) on [0, w_max]
         python gen_h_poly.py L <degree>                1 - log2(1+E) on E in [0, 1] (absolute error)
-        python gen_h_poly.py hs <w_max> <degree>       h rescaled for the packed FP32 kernel:
+        python gen_h_poly.py E2 <degree>               2^(-f) on f in [-1/2, 1/2] (relative error)
+        python gen_h_poly.py hs <w_max> <degree>       h rescaled for the packed FP32 / lean FP64 kernels:
                                                        h(w)/(4 log2 e) as a polynomial in w' = 4 (log2 e)^2 w
 Not imported by anything; the printed numbers were pasted into wl_field_device.cuh.
 Independent of oracle/ (which uses the Maclaurin series for u < 0.1).
@@ -28,9 +29,9 @@ def h(w):
     return (u * mp.tanh(u) - mp.log(mp.cosh(u))) / w
 
 
-def fit(w_max, deg, f=h):
+def fit(w_max, deg, f=h, lo=0):
     n = deg + 1
-    nodes = [(mp.cos(mp.pi * (2 * k + 1) / (2 * n)) + 1) / 2 * w_max for k in range(n)]
+    nodes = [(mp.cos(mp.pi * (2 * k + 1) / (2 * n)) + 1) / 2 * (w_max - lo) + lo for k in range(n)]
     A = mp.matrix(n, n)
     b = mp.matrix(n, 1)
     for r, x in enumerate(nodes):
@@ -80,7 +81,22 @@ if __name__ == "__main__":
         print("// max abs. error: exact coefficients %s, float32 coefficients %s"
               % (mp.nstr(max_abs_err(coef, 1, L, lambda c: c), 3), mp.nstr(max_abs_err(coef, 1, L, f32), 3)))
         for i, c in enumerate(coef):
-            print("c%d = %s" % (i, mp.nstr(c, 12)))
+            print("c%d = %s" % (i, mp.nstr(c, 20)))
+        sys.exit(0)
+    if sys.argv[1] == "E2":
+        deg = int(sys.argv[2])
+        f = lambda x: mp.power(2, -x)
+        coef = fit(mp.mpf(1) / 2, deg, f, lo=-mp.mpf(1) / 2)
+        worst = mp.mpf(0)
+        for k in range(2001):
+            x = -mp.mpf(1) / 2 + mp.mpf(k) / 2000
+            acc = mp.mpf(0)
+            for c in reversed(coef):
+                acc = acc * x + c
+            worst = max(worst, abs(acc / f(x) - 1))
+        print("// 2^(-f), f in [-1/2, 1/2], degree %d, max rel. error %s" % (deg, mp.nstr(worst, 3)))
+        for i, c in enumerate(coef):
+            print("c%d = %s" % (i, mp.nstr(c, 20)))
         sys.exit(0)
     if sys.argv[1] == "hs":
         w_max, deg = float(sys.argv[2]), int(sys.argv[3])
@@ -92,7 +108,7 @@ if __name__ == "__main__":
         print("// max rel. error of h: exact coefficients %s, float32 coefficients %s"
               % (mp.nstr(max_rel_err(coef, w_max, lambda c: c), 3), mp.nstr(max_rel_err(coef, w_max, f32), 3)))
         for i, c in enumerate(sc):
-            print("c%d = %s" % (i, mp.nstr(c, 12)))
+            print("c%d = %s" % (i, mp.nstr(c, 20)))
         sys.exit(0)
     w_max = float(sys.argv[1])
     deg = int(sys.argv[2])

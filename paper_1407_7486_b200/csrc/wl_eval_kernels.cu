@@ -248,6 +248,8 @@ cudaError_t launch_wilson(const EvalPlan& plan, const EvalArgs& a, int profile, 
         if (p2.P < 2) { p2.P = 2; p2.n_tiles = (p2.n_grid + kThreads * 2 - 1) / (kThreads * 2); }
         return launch_wilson_sech2_f32(p2, a, s);
     }
+    if (compute == WL_F64 && profile == WL_PROFILE_SECH2 && a.phi == nullptr)
+        return launch_wilson_sech2_f64(plan, a, s);
     return compute == WL_F32 ? launch_r<float>(plan, a, profile, s) : launch_r<double>(plan, a, profile, s);
 }
 

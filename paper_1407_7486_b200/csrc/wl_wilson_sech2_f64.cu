@@ -1,0 +1,240 @@
+// wl_wilson_sech2_f64.cu -- k_wilson_sech2_f64: the FP64 hot loop for the sech^2 profile with x_cm on
+// the x axis (phi_cm = NULL): configs 1 and 4 (FP64 variant) of BASELINE.json.  CUDA path, sm_100a.
+// Same mapping, summation order and epilogue as the generic k_wilson<double, Sech2, ...>; what differs is
+// that every elementary function is written out branch-free for the FP64 pipe (64 lanes/clk/SM, DFMA
+// = 2 clk per warp instruction per sub-partition, profiles/r01_pipe_rates.md) instead of calling the
+// general-purpose exp / log1p / sqrt / division sequences (~200 FP64-pipe instructions per point-eval
+// with slow-path branches):
+//
+//   sqrt, 1/w : MUFU.RSQ64H seed + two coupled Newton (Goldschmidt) steps + one residual correction
+//   2^(-u)    : round-to-nearest split u = n + f via the 1.5*2^52 trick, degree-10 polynomial in f,
+//               exponent adjusted with integer adds (E = exp(-2 rho/lambda) = 2^(-u'), u' = sqrt(w'))
+//   1/((1+E_p)(1+E_m)) : ONE MUFU.RCP64H seed + two Newton steps, shared by point and midpoint
+//   1 - log2(1+E_m)    : degree-20 polynomial in E_m in [0,1]
+//   near the axis (u^2 < 1/16): degree-7 polynomial in w' for the cancelling bracket (reading A4)
+// about 100 FP64-pipe instructions per point-eval.  Coefficients: gen_h_poly.py (E2 10, L 20, hs 0.0625 7).
+// Scaling as in wl_wilson_sech2_f32.cu: all squared radii carried as w' = (2 log2(e)/lambda)^2 w.
+#include "wl_internal.cuh"
+
+namespace wl {
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kChunk = 512;        // loop points staged in shared memory at a time (48 B each)
+
+__device__ __forceinline__ double xu_rsqrt64(double x) { double y; asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x)); return y; }
+__device__ __forceinline__ double xu_rcp64(double x) { double y; asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x)); return y; }
+
+// s = sqrt(w), ir = 1/sqrt(w) for w > 0 (w >= 1e-300): seed ~2^-22, two coupled steps -> ~2^-88, then
+// one residual step on s.  9 FP64-pipe instructions + 1 MUFU.
+__device__ __forceinline__ void sqrt_rsqrt(double w, double& s, double& ir)
+{
+    const double r0 = xu_rsqrt64(w);
+    double g = w * r0;                 // -> sqrt(w)
+    double h = 0.5 * r0;               // -> 1/(2 sqrt(w))
+    double e = fma(-g, h, 0.5);
+    g = fma(g, e, g);
+    h = fma(h, e, h);
+    e = fma(-g, h, 0.5);
+    g = fma(g, e, g);
+    h = fma(h, e, h);
+    const double d = fma(-g, g, w);    // residual
+    s = fma(d, h, g);
+    ir = h + h;
+}
+
+// 2^(-u) for u >= 0.  u = n + f, n = rint(u), |f| <= 1/2; 2^(-f) by a degree-10 polynomial (rel. error
+// 3e-16); 2^(-n) by subtracting n from the exponent field (n clamped to 1000: the result is then < 1e-301).
+__device__ __forceinline__ double exp2_neg(double u)
+{
+    const double kMagic = 6755399441055744.0;            // 1.5 * 2^52
+    const double t = u + kMagic;
+    const double f = u - (t - kMagic);
+    double p = 7.0725859492692236999e-9;
+    p = fma(p, f, -1.0208690299958305835e-7);
+    p = fma(p, f, 1.3215442587921689653e-6);
+    p = fma(p, f, -0.000015252657260200837064);
+    p = fma(p, f, 0.00015403530441736050155);
+    p = fma(p, f, -0.0013333558230164973899);
+    p = fma(p, f, 0.0096181291076068885273);
+    p = fma(p, f, -0.055504108664447719166);
+    p = fma(p, f, 0.2402265069591009822);
+    p = fma(p, f, -0.69314718055994998286);
+    p = fma(p, f, 1.0);
+    const int n = min(__double2loint(t), 1000);
+    return __hiloint2double(__double2hiint(p) - (n << 20), __double2loint(p));
+}
+
+// 1 - log2(1+E), E in [0,1]: degree-20 polynomial (abs. error 2e-17 + rounding).
+__device__ __forceinline__ double one_minus_log2_1p(double E)
+{
+    double L = 0.000037716935465554877791;
+    L = fma(L, E, -0.00043656761569165172581);
+    L = fma(L, E, 0.0024001133617501894281);
+    L = fma(L, E, -0.0083829321823817315509);
+    L = fma(L, E, 0.021049247229017102326);
+    L = fma(L, E, -0.040925999935882766517);
+    L = fma(L, E, 0.065142917694358537062);
+    L = fma(L, E, -0.089143555615740867799);
+    L = fma(L, E, 0.10983761672477964967);
+    L = fma(L, E, -0.12712681926472003036);
+    L = fma(L, E, 0.14301332675890233011);
+    L = fma(L, E, -0.15998872460281850448);
+    L = fma(L, E, 0.1802769786868982234);
+    L = fma(L, E, -0.20609048918280538869);
+    L = fma(L, E, 0.24044821605097346373);
+    L = fma(L, E, -0.28853893413338524963);
+    L = fma(L, E, 0.360673756378019119);
+    L = fma(L, E, -0.4808983468401831136);
+    L = fma(L, E, 0.72134752044239441043);
+    L = fma(L, E, -1.4426950408889492514);
+    L = fma(L, E, 0.99999999999999998397);
+    return L;
+}
+
+}  // namespace
+
+template <int P>
+__global__ void __launch_bounds__(kThreads, 2)
+k_wilson_sech2_f64(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double2* sPt = reinterpret_cast<double2*>(smem_raw);      // (y_x, |y|^2)
+    double2* sMid = sPt + kChunk;                             // (ybar_x, |ybar|^2)
+    double2* sCr = sMid + kChunk;                             // (dy_y/2, y_i x y_{i+1})
+
+    const int tid = threadIdx.x;
+    const int tile = blockIdx.x % n_tiles;
+    const int64_t unit = blockIdx.x / n_tiles;
+    const int N = a.n_ppl;
+    const double eB0 = a.p0, lambda = a.p1;
+    const double k = 2.0 * 1.4426950408889634074 / lambda;
+    const double k2 = k * k;
+
+    double R2[P], ax[P], Tt[P];
+    int gp[P];
+#pragma unroll
+    for (int j = 0; j < P; ++j) {
+        gp[j] = tile * (kThreads * P) + j * kThreads + tid;
+        const int g = min(gp[j], n_grid - 1);
+        const double T = a.T[g / a.n_rho];
+        const double rho = a.rho[g % a.n_rho];
+        R2[j] = k2 * rho * rho;
+        ax[j] = k2 * 2.0 * sqrt(T) * rho;
+        Tt[j] = k2 * T;
+    }
+    constexpr double kTiny = 1e-300;
+    constexpr double kPolyBelow = 0.52034224525;         // w' < this  <=>  u^2 < 1/16
+
+    double Wsum[P];
+#pragma unroll
+    for (int j = 0; j < P; ++j) Wsum[j] = 0.0;
+
+    for (int ll = 0; ll < loops_per_unit; ++ll) {
+        const int64_t loop = unit * loops_per_unit + ll;
+        const double2* L64 = reinterpret_cast<const double2*>(a.loops) + loop * N;
+        const float2* L32 = reinterpret_cast<const float2*>(a.loops) + loop * N;
+        double ph[P], sp[P];
+#pragma unroll
+        for (int j = 0; j < P; ++j) { ph[j] = 0.0; sp[j] = 0.0; }
+
+        for (int c0 = 0; c0 < N; c0 += kChunk) {
+            const int cn = min(kChunk, N - c0);
+            __syncthreads();                                  // the previous chunk has been consumed
+            for (int i = tid; i < cn; i += kThreads) {        // stage: derived unit-loop quantities
+                const int n = c0 + i;
+                const int n1 = (n + 1 == N) ? 0 : n + 1;      // closed loop, i+1 mod N
+                double yx, yy, zx, zy;
+                if (a.loops_are_f64) {
+                    const double2 u = L64[n], v = L64[n1];
+                    yx = u.x; yy = u.y; zx = v.x; zy = v.y;
+                } else {
+                    const float2 u = L32[n], v = L32[n1];
+                    yx = u.x; yy = u.y; zx = v.x; zy = v.y;
+                }
+                const double mx = 0.5 * (yx + zx), my = 0.5 * (yy + zy);
+                sPt[i] = make_double2(yx, yx * yx + yy * yy);
+                sMid[i] = make_double2(mx, mx * mx + my * my);
+                sCr[i] = make_double2(0.5 * (zy - yy), yx * zy - yy * zx);
+            }
+            __syncthreads();
+
+            for (int i = 0; i < cn; ++i) {
+                const double2 pt = sPt[i];
+                const double2 md = sMid[i];
+                const double2 cx = sCr[i];
+#pragma unroll
+                for (int j = 0; j < P; ++j) {
+                    // |x_i|^2 and |m_i|^2 (times k^2): eq. (8), (25)-(28)
+                    const double wp = fabs(fma(Tt[j], pt.y, fma(ax[j], pt.x, R2[j]))) + kTiny;
+                    const double wm = fabs(fma(Tt[j], md.y, fma(ax[j], md.x, R2[j]))) + kTiny;
+                    double up, irp, um, irm;
+                    sqrt_rsqrt(wp, up, irp);
+                    sqrt_rsqrt(wm, um, irm);
+                    (void)irp;
+                    const double Ep = exp2_neg(up), Em = exp2_neg(um);
+                    const double Dp = 1.0 + Ep, Dm = 1.0 + Em;
+                    const double DD = Dp * Dm;
+                    double r = xu_rcp64(DD);                                  // 1/((1+E_p)(1+E_m))
+                    double e = fma(-DD, r, 1.0);
+                    r = fma(r, e, r);
+                    e = fma(-DD, r, 1.0);
+                    r = fma(r, e, r);
+                    const double ip = r * Dm, im = r * Dp;
+                    sp[j] = fma(Ep * ip, ip, sp[j]);                          // E_p/(1+E_p)^2 = sech^2/4
+                    const double br = fma(-um, Em * im, one_minus_log2_1p(Em));   // (1 - log2(1+E_m)) - u' E_m/(1+E_m)
+                    const double hE = br * (irm * irm);                       // br / w'
+                    // h(w)/(4 log2 e) in w', w = u^2 < 1/16 (gen_h_poly.py hs 0.0625 7)
+                    double hP = -7.7102839224224163556e-11;
+                    hP = fma(hP, wm, 1.7289132522207449606e-9);
+                    hP = fma(hP, wm, -3.519550981355539808e-8);
+                    hP = fma(hP, wm, 7.0992077974390822073e-7);
+                    hP = fma(hP, wm, -0.000014180275863490838682);
+                    hP = fma(hP, wm, 0.00027778246137776088779);
+                    hP = fma(hP, wm, -0.0052035101873268705174);
+                    hP = fma(hP, wm, 0.086643397569993163057);
+                    const double gt = (wm < kPolyBelow) ? hP : hE;
+                    const double cr = fma(ax[j], cx.x, Tt[j] * cx.y);         // k^2 (m x d), eq. (24)
+                    ph[j] = fma(gt, cr, ph[j]);
+                }
+            }
+        }
+
+        // ---- W = cos(phase) cosh(spin), once per (loop, grid point): eq. (18), PAPER.md:121 ----
+        const double g_scale = eB0 * lambda * lambda * 0.69314718055994530942;
+        const double b_scale = 4.0 * eB0;
+#pragma unroll
+        for (int j = 0; j < P; ++j) {
+            const int g = min(gp[j], n_grid - 1);
+            const double T = a.T[g / a.n_rho];
+            const double phase = g_scale * ph[j];
+            const double spin = b_scale * (T / double(N)) * sp[j];
+            const double W = a.scalar ? cos(phase) : cos(phase) * cosh(spin);
+            Wsum[j] += W;
+            if (gp[j] < n_grid) {
+                if (a.phase_out) a.phase_out[loop * n_grid + gp[j]] = phase;
+                if (a.spin_out) a.spin_out[loop * n_grid + gp[j]] = spin;
+            }
+        }
+    }
+#pragma unroll
+    for (int j = 0; j < P; ++j)
+        if (gp[j] < n_grid) a.partial[unit * n_grid + gp[j]] = Wsum[j];
+}
+
+cudaError_t launch_wilson_sech2_f64(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s)
+{
+    const size_t smem = 3 * sizeof(double2) * (size_t)kChunk;
+    const int64_t n_ctas = plan.n_units * plan.n_tiles;
+    if (n_ctas > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    const unsigned g = (unsigned)n_ctas;
+    switch (plan.P) {
+        case 1: k_wilson_sech2_f64<1><<<g, kThreads, smem, s>>>(a, plan.n_grid, plan.n_tiles, plan.loops_per_unit); break;
+        case 2: k_wilson_sech2_f64<2><<<g, kThreads, smem, s>>>(a, plan.n_grid, plan.n_tiles, plan.loops_per_unit); break;
+        default: return cudaErrorInvalidValue;
+    }
+    return cudaGetLastError();
+}
+
+}  // namespace wl
