@@ -203,6 +203,87 @@ int wlo_eval_particle(int profile, const double *params, int scalar,
 }
 
 /* ------------------------------------------------------------------------- */
+/* Discretisation estimate, Sec. IV.A, eq. (48)-(52).       */
+/* Each N-point worldline is divided into three interleaved sub-worldlines    */
+/* (Fig. 2): "circle" = every other point (N/2 points: 0, 2, 4, ...), and the */
+/* remaining points split alternately into "box" (1, 5, 9, ...) and           */
+/* "triangle" (3, 7, 11, ...), N/4 points each; every sub-worldline is closed */
+/* on itself and evaluated as a loop of its own (same T, same x_cm;           */
+/* a sub-loop of a d-loop has the prescribed distribution).     */
+/* With I = the worldline integral of a sub-worldline:                        */
+/*   level 0:  <W>_{N/4} = < e^{i I_tri/2} e^{i I_box/2} >              (48)  */
+/*   level 1:  <W>_{N/2} = < e^{i I_circ} >                             (49)  */
+/*   level 2:  <W>_{N}   = < e^{i I_circ/2} e^{i I_box/4} e^{i I_tri/4} > (50) */
+/* Real part only (reading A5); for a fermion loop the spin integrals of the  */
+/* sub-worldlines are combined with the same weights (reading A15). */
+/*   group_sums3 [3][G][n_T][n_rho]; W3_loop nullable [3][n_loops][n_T][n_rho] */
+/* N must be a multiple of 4.  Returns 0 or -1.                               */
+/* ------------------------------------------------------------------------- */
+int wlo_eval_discretization(int profile, const double *params, int scalar,
+                            const double *loops, int64_t n_loops, int N,
+                            const double *T, int n_T,
+                            const double *rho_cm, const double *phi_cm, int n_rho,
+                            int n_groups, double *group_sums3, double *W3_loop)
+{
+    if (n_loops <= 0 || N < 4 || N % 4 != 0 || n_T < 1 || n_rho < 1 || n_groups < 1) return -1;
+    if (n_loops % n_groups != 0) return -1;
+    const int64_t n_grid = (int64_t)n_T * n_rho;
+    const int64_t per_group = n_loops / n_groups;
+    double *W = W3_loop ? W3_loop : (double *)malloc(sizeof(double) * 3 * n_loops * n_grid);
+    if (!W) return -1;
+    int fail = 0;
+
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t l = 0; l < n_loops; ++l) {
+        const double *y = loops + l * (int64_t)N * 2;
+        double *circ = (double *)malloc(sizeof(double) * N * 2);   /* N/2 + N/4 + N/4 points */
+        if (!circ) { fail = 1; continue; }
+        double *box = circ + N, *tri = box + N / 2;
+        for (int q = 0; q < N / 2; ++q) { circ[2 * q] = y[2 * (2 * q)]; circ[2 * q + 1] = y[2 * (2 * q) + 1]; }
+        for (int q = 0; q < N / 4; ++q) {
+            box[2 * q] = y[2 * (4 * q + 1)]; box[2 * q + 1] = y[2 * (4 * q + 1) + 1];
+            tri[2 * q] = y[2 * (4 * q + 3)]; tri[2 * q + 1] = y[2 * (4 * q + 3) + 1];
+        }
+        for (int t = 0; t < n_T; ++t)
+            for (int r = 0; r < n_rho; ++r) {
+                double ph = phi_cm ? phi_cm[r] : 0.0;
+                double cx = rho_cm[r] * cos(ph), cy = rho_cm[r] * sin(ph);
+                double Ic, Sc, Ib, Sb, It, St;
+                wlo_loop_phase_spin(profile, params, circ, N / 2, T[t], cx, cy, &Ic, &Sc);
+                wlo_loop_phase_spin(profile, params, box, N / 4, T[t], cx, cy, &Ib, &Sb);
+                wlo_loop_phase_spin(profile, params, tri, N / 4, T[t], cx, cy, &It, &St);
+                double phase[3] = { 0.5 * It + 0.5 * Ib, Ic, 0.5 * Ic + 0.25 * Ib + 0.25 * It };
+                double spin[3] = { 0.5 * St + 0.5 * Sb, Sc, 0.5 * Sc + 0.25 * Sb + 0.25 * St };
+                for (int lev = 0; lev < 3; ++lev)
+                    W[((int64_t)lev * n_loops + l) * n_grid + (int64_t)t * n_rho + r] =
+                        scalar ? cos(phase[lev]) : cos(phase[lev]) * cosh(spin[lev]);
+            }
+        free(circ);
+    }
+    if (!fail)
+        for (int lev = 0; lev < 3; ++lev)
+            for (int64_t k = 0; k < n_grid; ++k)
+                for (int g = 0; g < n_groups; ++g) {
+                    double S = 0.0;
+                    for (int64_t l = g * per_group; l < (g + 1) * per_group; ++l)
+                        S += W[((int64_t)lev * n_loops + l) * n_grid + k];
+                    group_sums3[((int64_t)lev * n_groups + g) * n_grid + k] = S;
+                }
+    if (!W3_loop) free(W);
+    return fail ? -1 : 0;
+}
+
+/* eq. (51)-(52): parabola through the three levels in 1/N.  */
+void wlo_extrapolate(const double *lev3, int64_t n, double *W_inf, double *delta)
+{
+    for (int64_t k = 0; k < n; ++k) {
+        double w4 = lev3[k], w2 = lev3[n + k], w1 = lev3[2 * n + k];
+        W_inf[k] = 8.0 / 3.0 * w1 - 2.0 * w2 + 1.0 / 3.0 * w4;
+        if (delta) delta[k] = fabs(w1 - W_inf[k]);
+    }
+}
+
+/* ------------------------------------------------------------------------- */
 /* Jackknife finalise, eq. (60)-(63); delete-one-group means (reading A7).    */
 /*   mean, err [n_grid]; delete_one nullable [G][n_grid]                      */
 /* ------------------------------------------------------------------------- */

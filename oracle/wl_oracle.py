@@ -38,6 +38,11 @@ def lib():
         L.wlo_eval_particle.restype = C.c_int
         L.wlo_eval_particle.argtypes = [C.c_int, _dp, C.c_int, _dp, C.c_int64, C.c_int, _dp, C.c_int, _dp, _dp,
                                         C.c_int, C.c_int, _dp, _dp, _dp, _dp, _dp]
+        L.wlo_eval_discretization.restype = C.c_int
+        L.wlo_eval_discretization.argtypes = [C.c_int, _dp, C.c_int, _dp, C.c_int64, C.c_int, _dp, C.c_int, _dp,
+                                              _dp, C.c_int, C.c_int, _dp, _dp]
+        L.wlo_extrapolate.restype = None
+        L.wlo_extrapolate.argtypes = [_dp, C.c_int64, _dp, _dp]
         L.wlo_finalize.restype = C.c_int
         L.wlo_finalize.argtypes = [_dp, C.c_int, C.c_int64, C.c_int64, _dp, _dp, _dp]
         L.wlo_philox4x32_10.restype = None
@@ -114,6 +119,36 @@ def evaluate(profile, params, loops, T, rho_cm, phi_cm=None, n_groups=1, per_loo
     if per_loop:
         out.update(W=W, phase=ph, spin=sp)
     return out
+
+
+def evaluate_discretization(profile, params, loops, T, rho_cm, phi_cm=None, n_groups=1, per_loop=False,
+                            scalar=False):
+    """Sec. IV.A, eq. (48)-(50): group sums [3][G][n_T][n_rho] at the levels (N/4, N/2, N) of the paper's
+    interleaved sub-worldline scheme (and per-loop W [3][n_loops][n_T][n_rho] if per_loop)."""
+    pr = _f64(params)
+    y = _f64(loops)
+    assert y.ndim == 3 and y.shape[2] == 2
+    T = _f64(T)
+    rho = _f64(rho_cm)
+    phi = _f64(phi_cm) if phi_cm is not None else None
+    nl, N = y.shape[0], y.shape[1]
+    gs = np.empty((3, n_groups, T.shape[0], rho.shape[0]))
+    W = np.empty((3, nl, T.shape[0], rho.shape[0])) if per_loop else None
+    rc = lib().wlo_eval_discretization(profile, _p(pr), 1 if scalar else 0, _p(y), nl, N, _p(T), T.shape[0],
+                                       _p(rho), _p(phi), rho.shape[0], n_groups, _p(gs), _p(W))
+    if rc != 0:
+        raise ValueError("wlo_eval_discretization: invalid argument (N must be a multiple of 4)")
+    return (gs, W) if per_loop else gs
+
+
+def extrapolate(levels):
+    """eq. (51)-(52): levels [3][...] (N/4, N/2, N) -> (W_inf, delta = |W_N - W_inf|)."""
+    a = _f64(levels)
+    n = int(np.prod(a.shape[1:])) if a.ndim > 1 else 1
+    out = np.empty(n)
+    delta = np.empty(n)
+    lib().wlo_extrapolate(_p(a), n, _p(out), _p(delta))
+    return out.reshape(a.shape[1:]), delta.reshape(a.shape[1:])
 
 
 def finalize(group_sums, n_loops, delete_one=False):
