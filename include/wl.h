@@ -145,6 +145,30 @@ wl_status wl_eval_per_loop(const wl_field* field,
                            wl_dtype compute,
                            double* d_W, double* d_phase, double* d_spin, void* stream);
 
+/* Discretisation estimate, Sec. IV.A, eq. (48)-(52), PAPER.md:269-304 (reading A15).
+ * Every N-point loop is divided into three interleaved sub-worldlines, each closed on itself:
+ * "circle" = points 0, 2, 4, ... (N/2 points), "box" = 1, 5, 9, ..., "triangle" = 3, 7, 11, ...
+ * (N/4 points each).  With I the worldline integral (phase) of a sub-worldline,
+ *   level 0 (N/4): W = cos(I_tri/2 + I_box/2)                 eq. (48)
+ *   level 1 (N/2): W = cos(I_circ)                            eq. (49)
+ *   level 2 (N)  : W = cos(I_circ/2 + I_box/4 + I_tri/4)      eq. (50)
+ * times, for a fermion field, cosh of the sub-worldlines' spin integrals combined with the same weights.
+ * Writes d_group_sums3[3][n_groups][n_T][n_rho] (levels N/4, N/2, N), in the fixed order of wl_eval.
+ * n_ppl must be a multiple of 4 (else WL_ERR_INVALID_ARG).  Other arguments and errors as wl_eval;
+ * the workspace size is wl_eval_discretization_workspace_bytes (0 on invalid sizes). */
+size_t wl_eval_discretization_workspace_bytes(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups,
+                                              wl_dtype compute);
+wl_status wl_eval_discretization(const wl_field* field,
+                                 const void* d_loops, wl_dtype loop_dtype, int64_t n_loops, int n_ppl,
+                                 const double* d_T, int n_T,
+                                 const double* d_rho_cm, const double* d_phi_cm, int n_rho,
+                                 int n_groups, wl_dtype compute, double* d_group_sums3,
+                                 void* d_workspace, size_t workspace_bytes, void* stream);
+
+/* eq. (51)-(52), element-wise on d_levels3[3][n] (levels N/4, N/2, N: means or group sums):
+ *   d_W_inf[k] = 8/3 W_N - 2 W_{N/2} + 1/3 W_{N/4},   d_delta[k] = |W_N - W_inf|  (d_delta may be NULL). */
+wl_status wl_extrapolate(const double* d_levels3, int64_t n, double* d_W_inf, double* d_delta, void* stream);
+
 /* Jackknife finalise, eq. (60)-(63).  From d_group_sums[G][n_T][n_rho]:
  *   d_mean[t][r] = (sum_g S_g)/n_loops,
  *   d_err[t][r]  = sqrt(sum_g (S_g G/n_loops - mean)^2 / (G (G-1))),

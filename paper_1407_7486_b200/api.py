@@ -46,6 +46,13 @@ _lib.wl_eval.argtypes = [_vp, _vp, _int, _i64, _int, _dp, _int, _dp, _dp, _int, 
                          _vp, _sz, _vp]
 _lib.wl_eval_instrumented.restype = _int
 _lib.wl_eval_instrumented.argtypes = list(_lib.wl_eval.argtypes) + [_vp, _vp]
+_lib.wl_eval_discretization_workspace_bytes.restype = _sz
+_lib.wl_eval_discretization_workspace_bytes.argtypes = [_i64, _int, _int, _int, _int, _int]
+_lib.wl_eval_discretization.restype = _int
+_lib.wl_eval_discretization.argtypes = [_vp, _vp, _int, _i64, _int, _dp, _int, _dp, _dp, _int, _int, _int, _dp,
+                                        _vp, _sz, _vp]
+_lib.wl_extrapolate.restype = _int
+_lib.wl_extrapolate.argtypes = [_dp, _i64, _dp, _dp, _vp]
 _lib.wl_eval_per_loop.restype = _int
 _lib.wl_eval_per_loop.argtypes = [_vp, _vp, _int, _i64, _int, _dp, _int, _dp, _dp, _int, _int, _dp, _dp,
                                   _dp, _vp]
@@ -208,6 +215,37 @@ def wl_eval(field, loops, T, rho_cm, phi_cm=None, n_groups=1, compute=torch.floa
             e0, e1 = (_event_handle(ev, stream) for ev in wilson_events)
             _check(_lib.wl_eval_instrumented(*args, _stream(stream), e0, e1), "wl_eval_instrumented")
     return W_mean, group_sums
+
+
+def wl_eval_discretization(field, loops, T, rho_cm, phi_cm=None, n_groups=1, compute=torch.float64, stream=None):
+    """Group sums [3][G][n_T][n_rho] at the levels (N/4, N/2, N) of Sec. IV.A, eq. (48)-(50)."""
+    n_loops, n_ppl = _loops_arg(loops)
+    T = _cuda_f64(T, "T")
+    rho_cm = _cuda_f64(rho_cm, "rho_cm")
+    n_T, n_rho = T.numel(), rho_cm.numel()
+    phi_cm = _cuda_f64(phi_cm, "phi_cm", n_rho)
+    cc = _dtype_code(compute)
+    gs3 = torch.empty((3, n_groups, n_T, n_rho), dtype=torch.float64, device=loops.device)
+    need = int(_lib.wl_eval_discretization_workspace_bytes(n_loops, n_ppl, n_T, n_rho, n_groups, cc))
+    ws = torch.empty(max(need, 8), dtype=torch.uint8, device=loops.device)
+    with torch.cuda.device(loops.device):
+        _check(_lib.wl_eval_discretization(field._h, _ptr(loops), _dtype_code(loops.dtype), n_loops, n_ppl, _ptr(T),
+                                           n_T, _ptr(rho_cm), _ptr(phi_cm), n_rho, int(n_groups), cc, _ptr(gs3),
+                                           _ptr(ws), need, _stream(stream)), "wl_eval_discretization")
+    return gs3
+
+
+def wl_extrapolate(levels3, want_delta=True, stream=None):
+    """eq. (51)-(52) element-wise on levels3 [3][...] -> (W_inf, delta)."""
+    lv = _cuda_f64(levels3, "levels3")
+    if lv.shape[0] != 3:
+        raise ValueError("levels3 must be [3][...]")
+    n = lv.numel() // 3
+    out = torch.empty(lv.shape[1:], dtype=torch.float64, device=lv.device)
+    delta = torch.empty_like(out) if want_delta else None
+    with torch.cuda.device(lv.device):
+        _check(_lib.wl_extrapolate(_ptr(lv), n, _ptr(out), _ptr(delta), _stream(stream)), "wl_extrapolate")
+    return out, delta
 
 
 def wl_eval_per_loop(field, loops, T, rho_cm, phi_cm=None, compute=torch.float64, want_phase_spin=True,

@@ -107,7 +107,7 @@ wl_status wl_eval_instrumented(const wl_field* field, const void* d_loops, wl_dt
     EvalArgs a;
     a.loops = d_loops; a.loops_are_f64 = (loop_dtype == WL_F64); a.n_loops = n_loops; a.n_ppl = n_ppl;
     a.T = d_T; a.rho = d_rho_cm; a.phi = d_phi_cm; a.n_T = n_T; a.n_rho = n_rho;
-    a.p0 = field->p0; a.p1 = field->p1; a.scalar = field->scalar;
+    a.p0 = field->p0; a.p1 = field->p1; a.scalar = field->scalar; a.disc = 0;
     a.partial = reinterpret_cast<double*>(d_workspace);
     a.phase_out = nullptr; a.spin_out = nullptr;
     cudaStream_t s = (cudaStream_t)stream;
@@ -117,6 +117,66 @@ wl_status wl_eval_instrumented(const wl_field* field, const void* d_loops, wl_dt
     if (event_wilson_end && cudaEventRecord((cudaEvent_t)event_wilson_end, s) != cudaSuccess) return WL_ERR_CUDA;
     e = launch_group_reduce(a.partial, plan.n_units, plan.units_per_group, n_groups, plan.n_grid, n_loops,
                             d_group_sums, d_W_mean, s);
+    return e == cudaSuccess ? WL_OK : WL_ERR_CUDA;
+}
+
+namespace {
+
+// Plan of the discretisation run: the plan of an ordinary run over N/2 terms per pass, with at most
+// two grid points per thread (each carries three running W sums).
+EvalPlan make_disc_plan(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups, wl_dtype compute)
+{
+    EvalPlan p = make_eval_plan(n_loops, n_ppl / 2, n_T, n_rho, n_groups, compute, false);
+    if (p.P > 2) { p.P = 2; p.n_tiles = (p.n_grid + p.threads * 2 - 1) / (p.threads * 2); }
+    return p;
+}
+
+}  // namespace
+
+size_t wl_eval_discretization_workspace_bytes(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups,
+                                              wl_dtype compute)
+{
+    if (!sizes_ok(n_loops, n_ppl, n_T, n_rho, n_groups) || !dtype_ok(compute)) return 0;
+    if (n_ppl < 4 || n_ppl % 4 != 0) return 0;
+    const EvalPlan p = make_disc_plan(n_loops, n_ppl, n_T, n_rho, n_groups, compute);
+    return 3 * (size_t)p.n_units * (size_t)p.n_grid * sizeof(double);
+}
+
+wl_status wl_eval_discretization(const wl_field* field, const void* d_loops, wl_dtype loop_dtype,
+                                 int64_t n_loops, int n_ppl, const double* d_T, int n_T,
+                                 const double* d_rho_cm, const double* d_phi_cm, int n_rho, int n_groups,
+                                 wl_dtype compute, double* d_group_sums3, void* d_workspace,
+                                 size_t workspace_bytes, void* stream)
+{
+    if (!field || !d_loops || !d_T || !d_rho_cm || !d_group_sums3) return WL_ERR_INVALID_ARG;
+    if (!dtype_ok(loop_dtype) || !dtype_ok(compute)) return WL_ERR_INVALID_ARG;
+    if (!sizes_ok(n_loops, n_ppl, n_T, n_rho, n_groups)) return WL_ERR_INVALID_ARG;
+    if (n_ppl < 4 || n_ppl % 4 != 0) return WL_ERR_INVALID_ARG;            // three interleaved sub-worldlines
+    const EvalPlan plan = make_disc_plan(n_loops, n_ppl, n_T, n_rho, n_groups, compute);
+    const size_t level = (size_t)plan.n_units * (size_t)plan.n_grid;
+    if (!d_workspace || workspace_bytes < 3 * level * sizeof(double)) return WL_ERR_WORKSPACE;
+
+    EvalArgs a;
+    a.loops = d_loops; a.loops_are_f64 = (loop_dtype == WL_F64); a.n_loops = n_loops; a.n_ppl = n_ppl;
+    a.T = d_T; a.rho = d_rho_cm; a.phi = d_phi_cm; a.n_T = n_T; a.n_rho = n_rho;
+    a.p0 = field->p0; a.p1 = field->p1; a.scalar = field->scalar; a.disc = 1;
+    a.partial = reinterpret_cast<double*>(d_workspace);
+    a.phase_out = nullptr; a.spin_out = nullptr;
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaError_t e = launch_wilson(plan, a, field->profile, compute, s);
+    if (e != cudaSuccess) return e == cudaErrorInvalidValue ? WL_ERR_UNSUPPORTED : WL_ERR_CUDA;
+    for (int lev = 0; lev < 3; ++lev) {
+        e = launch_group_reduce(a.partial + lev * level, plan.n_units, plan.units_per_group, n_groups, plan.n_grid,
+                                n_loops, d_group_sums3 + (size_t)lev * n_groups * plan.n_grid, nullptr, s);
+        if (e != cudaSuccess) return WL_ERR_CUDA;
+    }
+    return WL_OK;
+}
+
+wl_status wl_extrapolate(const double* d_levels3, int64_t n, double* d_W_inf, double* d_delta, void* stream)
+{
+    if (!d_levels3 || !d_W_inf || n < 1) return WL_ERR_INVALID_ARG;
+    cudaError_t e = launch_extrapolate(d_levels3, n, d_W_inf, d_delta, (cudaStream_t)stream);
     return e == cudaSuccess ? WL_OK : WL_ERR_CUDA;
 }
 
@@ -132,7 +192,7 @@ wl_status wl_eval_per_loop(const wl_field* field, const void* d_loops, wl_dtype 
     EvalArgs a;
     a.loops = d_loops; a.loops_are_f64 = (loop_dtype == WL_F64); a.n_loops = n_loops; a.n_ppl = n_ppl;
     a.T = d_T; a.rho = d_rho_cm; a.phi = d_phi_cm; a.n_T = n_T; a.n_rho = n_rho;
-    a.p0 = field->p0; a.p1 = field->p1; a.scalar = field->scalar;
+    a.p0 = field->p0; a.p1 = field->p1; a.scalar = field->scalar; a.disc = 0;
     a.partial = d_W; a.phase_out = d_phase; a.spin_out = d_spin;
     cudaError_t e = launch_wilson(plan, a, field->profile, compute, (cudaStream_t)stream);
     if (e != cudaSuccess) return e == cudaErrorInvalidValue ? WL_ERR_UNSUPPORTED : WL_ERR_CUDA;

@@ -27,9 +27,18 @@ constexpr int kSumBlock = 32;     // FP32 partial sums span this many terms befo
 template <typename Real> struct alignas(16) Vec4 { Real a, b, c, d; };
 template <typename Real> struct alignas(2 * sizeof(Real)) Vec2 { Real a, b; };
 
-template <typename Real, template <typename> class Prof, bool HAS_PHI, int P>
+// DISC = true: the discretisation estimate of Sec. IV.A (eq. (48)-(50)).  Each loop is
+// walked as two VIRTUAL loops of N/2 terms: pass 0 = the even points with neighbour +2 (the "circle"
+// sub-worldline, N/2 points), pass 1 = the odd points with neighbour +4 (the "box" and "triangle"
+// sub-worldlines, N/4 points each, summed together).  With S2, S4 the phase sums and B2, B4 the spin
+// sums of the two passes, the three levels are
+//   N/4: phase = S4/2,          spin = 2 (T/N) B4      (mean of the two N/4 sub-worldlines)
+//   N/2: phase = S2,            spin = 2 (T/N) B2
+//   N  : phase = S2/2 + S4/4,   spin = (T/N)(B2 + B4)
+// and the partial sums are written level-major: partial[level][unit][grid].
+template <typename Real, template <typename> class Prof, bool HAS_PHI, int P, bool DISC>
 __global__ void __launch_bounds__(kThreads)
-k_wilson(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit, int chunk_points)
+k_wilson(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit, int chunk_points, int64_t n_units)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     Vec4<Real>* sSeg = reinterpret_cast<Vec4<Real>*>(smem_raw);            // (ybar_x, |ybar|^2, dy_y, y_i x y_{i+1})
@@ -62,24 +71,39 @@ k_wilson(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit, int chunk_poin
         if (HAS_PHI) { ay[j] = Real(2.0 * s * cy); scy[j] = Real(s * cy); }
     }
 
-    double Wsum[P];
+    constexpr int kLevels = DISC ? 3 : 1;
+    double Wsum[kLevels][P];
 #pragma unroll
-    for (int j = 0; j < P; ++j) Wsum[j] = 0.0;
+    for (int v = 0; v < kLevels; ++v)
+#pragma unroll
+        for (int j = 0; j < P; ++j) Wsum[v][j] = 0.0;
 
     for (int ll = 0; ll < loops_per_unit; ++ll) {
         const int64_t loop = unit * loops_per_unit + ll;
         const double2* L64 = reinterpret_cast<const double2*>(a.loops) + loop * N;
         const float2* L32 = reinterpret_cast<const float2*>(a.loops) + loop * N;
         double dph[P], dsp[P];
+        double S2[DISC ? P : 1], B2[DISC ? P : 1];       // pass-0 sums (DISC only)
 #pragma unroll
         for (int j = 0; j < P; ++j) { dph[j] = 0.0; dsp[j] = 0.0; }
 
-        for (int c0 = 0; c0 < N; c0 += chunk_points) {
-            const int cn = min(chunk_points, N - c0);
+      const int Nv = DISC ? N / 2 : N;                  // terms per pass
+      for (int pass = 0; pass < (DISC ? 2 : 1); ++pass) {
+        if (DISC && pass == 1) {
+#pragma unroll
+            for (int j = 0; j < P; ++j) { S2[j] = dph[j]; B2[j] = dsp[j]; dph[j] = 0.0; dsp[j] = 0.0; }
+        }
+        for (int c0 = 0; c0 < Nv; c0 += chunk_points) {
+            const int cn = min(chunk_points, Nv - c0);
             __syncthreads();                                  // the previous chunk has been consumed
             for (int i = tid; i < cn; i += kThreads) {        // stage: derived unit-loop quantities, FP64
-                const int n = c0 + i;
-                const int n1 = (n + 1 == N) ? 0 : n + 1;      // closed loop, i+1 mod N
+                int n = c0 + i;
+                int n1 = (n + 1 == N) ? 0 : n + 1;            // closed loop, i+1 mod N
+                if (DISC) {                                   // sub-worldline: every 2nd / 4th point, closed on itself
+                    n = pass + 2 * (c0 + i);
+                    n1 = n + (pass ? 4 : 2);
+                    if (n1 >= N) n1 -= N;
+                }
                 double yx, yy, zx, zy;
                 if (a.loops_are_f64) {
                     const double2 u = L64[n], v = L64[n1];
@@ -133,24 +157,38 @@ k_wilson(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit, int chunk_poin
             }
         }
 
+      }   // pass
+
         // ---- W = cos(phase) cosh(spin), FP64, once per (loop, grid point): eq. (18), PAPER.md:121 ----
 #pragma unroll
         for (int j = 0; j < P; ++j) {
             const int g = min(gp[j], n_grid - 1);
             const double T = a.T[g / a.n_rho];
-            const double phase = prof.g_scale() * dph[j];
-            const double spin = prof.b_scale() * (T / double(N)) * dsp[j];
-            const double W = a.scalar ? cos(phase) : cos(phase) * cosh(spin);
-            Wsum[j] += W;
-            if (gp[j] < n_grid) {
-                if (a.phase_out) a.phase_out[loop * n_grid + gp[j]] = phase;
-                if (a.spin_out) a.spin_out[loop * n_grid + gp[j]] = spin;
+            if (!DISC) {
+                const double phase = prof.g_scale() * dph[j];
+                const double spin = prof.b_scale() * (T / double(N)) * dsp[j];
+                const double W = a.scalar ? cos(phase) : cos(phase) * cosh(spin);
+                Wsum[0][j] += W;
+                if (gp[j] < n_grid) {
+                    if (a.phase_out) a.phase_out[loop * n_grid + gp[j]] = phase;
+                    if (a.spin_out) a.spin_out[loop * n_grid + gp[j]] = spin;
+                }
+            } else {
+                const double S4 = dph[j], B4 = dsp[j];
+                const double gs = prof.g_scale(), c = prof.b_scale() * (T / double(N));
+                const double phase[3] = {gs * (0.5 * S4), gs * S2[j], gs * (0.5 * S2[j] + 0.25 * S4)};   // eq. (48)-(50)
+                const double spin[3] = {2.0 * c * B4, 2.0 * c * B2[j], c * (B2[j] + B4)};
+#pragma unroll
+                for (int v = 0; v < 3; ++v)
+                    Wsum[v][j] += a.scalar ? cos(phase[v]) : cos(phase[v]) * cosh(spin[v]);
             }
         }
     }
 #pragma unroll
-    for (int j = 0; j < P; ++j)
-        if (gp[j] < n_grid) a.partial[unit * n_grid + gp[j]] = Wsum[j];
+    for (int v = 0; v < kLevels; ++v)
+#pragma unroll
+        for (int j = 0; j < P; ++j)
+            if (gp[j] < n_grid) a.partial[((int64_t)v * n_units + unit) * n_grid + gp[j]] = Wsum[v][j];
 }
 
 // S_g = sum over the units of group g, in unit order (eq. (60)).
@@ -205,25 +243,32 @@ EvalPlan make_eval_plan(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_gr
     return p;
 }
 
-template <typename Real, template <typename> class Prof, bool HAS_PHI, int P>
+template <typename Real, template <typename> class Prof, bool HAS_PHI, int P, bool DISC>
 static cudaError_t launch_one(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s)
 {
     const size_t per_point = sizeof(Vec4<Real>) + sizeof(Vec2<Real>) + (HAS_PHI ? sizeof(Vec4<Real>) : 0);
     const size_t smem = per_point * (size_t)plan.chunk_points;
     const int64_t n_ctas = plan.n_units * plan.n_tiles;
     if (n_ctas > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    k_wilson<Real, Prof, HAS_PHI, P><<<(unsigned)n_ctas, kThreads, smem, s>>>(
-        a, plan.n_grid, plan.n_tiles, plan.loops_per_unit, plan.chunk_points);
+    k_wilson<Real, Prof, HAS_PHI, P, DISC><<<(unsigned)n_ctas, kThreads, smem, s>>>(
+        a, plan.n_grid, plan.n_tiles, plan.loops_per_unit, plan.chunk_points, plan.n_units);
     return cudaGetLastError();
 }
 
 template <typename Real, template <typename> class Prof, bool HAS_PHI>
 static cudaError_t launch_p(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s)
 {
+    if (a.disc) {                                        // discretisation estimate: P <= 2 (three W per grid point)
+        switch (plan.P) {
+            case 1: return launch_one<Real, Prof, HAS_PHI, 1, true>(plan, a, s);
+            case 2: return launch_one<Real, Prof, HAS_PHI, 2, true>(plan, a, s);
+            default: return cudaErrorInvalidValue;
+        }
+    }
     switch (plan.P) {
-        case 1: return launch_one<Real, Prof, HAS_PHI, 1>(plan, a, s);
-        case 2: return launch_one<Real, Prof, HAS_PHI, 2>(plan, a, s);
-        case 4: if (sizeof(Real) == 4) return launch_one<Real, Prof, HAS_PHI, (sizeof(Real) == 4 ? 4 : 2)>(plan, a, s);
+        case 1: return launch_one<Real, Prof, HAS_PHI, 1, false>(plan, a, s);
+        case 2: return launch_one<Real, Prof, HAS_PHI, 2, false>(plan, a, s);
+        case 4: if (sizeof(Real) == 4) return launch_one<Real, Prof, HAS_PHI, (sizeof(Real) == 4 ? 4 : 2), false>(plan, a, s);
         default: return cudaErrorInvalidValue;
     }
 }
@@ -243,6 +288,8 @@ static cudaError_t launch_r(const EvalPlan& plan, const EvalArgs& a, int profile
 
 cudaError_t launch_wilson(const EvalPlan& plan, const EvalArgs& a, int profile, wl_dtype compute, cudaStream_t s)
 {
+    if (a.disc)
+        return compute == WL_F32 ? launch_r<float>(plan, a, profile, s) : launch_r<double>(plan, a, profile, s);
     if (compute == WL_F32 && profile == WL_PROFILE_SECH2 && a.phi == nullptr) {
         EvalPlan p2 = plan;                              // grid points go in register pairs there
         if (p2.P < 2) { p2.P = 2; p2.n_tiles = (p2.n_grid + kThreads * 2 - 1) / (kThreads * 2); }
@@ -262,6 +309,7 @@ cudaError_t launch_group_reduce(const double* partial, int64_t n_units, int unit
     k_group_reduce<<<grid, 256, 0, s>>>(partial, units_per_group, n_grid, group_sums);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
+    if (!W_mean) return cudaSuccess;
     k_mean<<<(n_grid + 255) / 256, 256, 0, s>>>(group_sums, n_groups, n_grid, (double)n_loops, W_mean);
     return cudaGetLastError();
 }

@@ -147,6 +147,26 @@ __global__ void k_jackknife_finalize(const double* __restrict__ group_sums, int 
     err[k] = sqrt(ss / (G * (G - 1.0)));                     // eq. (63)
 }
 
+// eq. (51)-(52): parabola in 1/N through the levels (N/4, N/2, N).
+__global__ void k_extrapolate(const double* __restrict__ lev3, int64_t n, double* __restrict__ W_inf,
+                              double* __restrict__ delta)
+{
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const double w4 = lev3[k], w2 = lev3[n + k], w1 = lev3[2 * n + k];
+    const double wi = 8.0 / 3.0 * w1 - 2.0 * w2 + 1.0 / 3.0 * w4;
+    W_inf[k] = wi;
+    if (delta) delta[k] = fabs(w1 - wi);
+}
+
+cudaError_t launch_extrapolate(const double* levels3, int64_t n, double* W_inf, double* delta, cudaStream_t s)
+{
+    const int64_t blocks = (n + 255) / 256;
+    if (blocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    k_extrapolate<<<(unsigned)blocks, 256, 0, s>>>(levels3, n, W_inf, delta);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_finalize(const double* group_sums, int n_groups, int64_t n_loops, int n_grid,
                             double* mean, double* err, double* delete_one, cudaStream_t s)
 {

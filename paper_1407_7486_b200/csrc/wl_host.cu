@@ -126,7 +126,7 @@ extern "C" wl_status wl_eval_host(const wl_field* field, const void* h_loops, wl
         a.loops = dst; a.loops_are_f64 = (loop_dtype == WL_F64); a.n_loops = nl; a.n_ppl = n_ppl;
         a.T = reinterpret_cast<const double*>(d.p[T]); a.rho = reinterpret_cast<const double*>(d.p[RHO]);
         a.phi = reinterpret_cast<const double*>(d.p[PHI]); a.n_T = n_T; a.n_rho = n_rho;
-        a.p0 = field->p0; a.p1 = field->p1; a.scalar = field->scalar;
+        a.p0 = field->p0; a.p1 = field->p1; a.scalar = field->scalar; a.disc = 0;
         a.partial = partial + (size_t)(l0 / plan.loops_per_unit) * plan.n_grid;
         a.phase_out = nullptr; a.spin_out = nullptr;
         cudaError_t e = wl::launch_wilson(sub, a, field->profile, compute, d.s);

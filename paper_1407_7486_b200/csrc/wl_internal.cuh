@@ -44,6 +44,7 @@ struct EvalArgs {
     int n_T, n_rho;
     double p0, p1;              // field parameters
     int scalar;                 // W = cos(phase) only
+    int disc;                   // discretisation estimate (three levels, generic kernel only)
     double* partial;            // [n_units][n_grid]
     double* phase_out;          // per-loop mode only, nullable
     double* spin_out;           // per-loop mode only, nullable
@@ -60,6 +61,7 @@ cudaError_t launch_group_reduce(const double* partial, int64_t n_units, int unit
                                 cudaStream_t s);
 cudaError_t launch_finalize(const double* group_sums, int n_groups, int64_t n_loops, int n_grid,
                             double* mean, double* err, double* delete_one, cudaStream_t s);
+cudaError_t launch_extrapolate(const double* levels3, int64_t n, double* W_inf, double* delta, cudaStream_t s);
 cudaError_t launch_generate(void* loops, int storage_is_f64, int64_t loop_begin, int64_t n_loops, int n_ppl,
                             uint64_t seed, cudaStream_t s);
 
