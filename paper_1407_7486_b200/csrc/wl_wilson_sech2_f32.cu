@@ -10,8 +10,9 @@
 //
 // So (i) the plain FP32 work is issued as PACKED fma/mul/add.f32x2 (FFMA2: two grid points per
 // instruction, one issue slot), every thread owning P grid points as P/2 register pairs; (ii) the
-// shared-memory copy of the loop holds every value twice, so that one LDS.128 yields two ready-made
-// packed operands; (iii) the special-function count per point-eval is 5 or 6:
+// staged loop values enter FFMA2 as both-halves scalar operands, so a staged point costs one LDS.128 and
+// one LDS.64 (shared-memory loads return through the same queue as the special-function results: every
+// 4 bytes per lane cost about one XU-pipe clock, profiles/r01_pipe_rates.md); (iii) the special-function count per point-eval is 5 or 6:
 //       sqrt(|x_i|^2), 2^(-u_p), rsqrt(|m_i|^2), 2^(-u_m), ONE reciprocal 1/((1+E_p)(1+E_m))
 //   and log2(1+E_m), the last either on the XU pipe (LOGPOLY = false) or as a degree-8 polynomial
 //   in E_m in [0,1] on the FMA pipe (LOGPOLY = true).
@@ -31,7 +32,7 @@ namespace {
 
 constexpr int kThreads = 256;
 constexpr int kSumBlock = 32;      // FP32 partial sums span this many terms before they go to FP64
-constexpr int kChunk = 512;        // loop points staged in shared memory at a time (48 B each)
+constexpr int kChunk = 1024;       // loop points staged in shared memory at a time (24 B each)
 
 typedef unsigned long long u64;    // two packed floats (lo, hi)
 
@@ -50,16 +51,15 @@ __device__ __forceinline__ float xu_lg2_abs(float x) { float y; asm("lg2.approx.
 
 }  // namespace
 
-template <int P, bool LOGPOLY, int MINB, int UNROLL, int SUMBLOCK>
-__global__ void __launch_bounds__(kThreads, MINB)
+template <int P, int THREADS, bool LOGPOLY, int MINB, int UNROLL, int SUMBLOCK>
+__global__ void __launch_bounds__(THREADS, MINB)
 k_wilson_sech2_f32(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit)
 {
     static_assert(P % 2 == 0, "grid points are processed as register pairs");
     constexpr int Q = P / 2;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    ulonglong2* sPt = reinterpret_cast<ulonglong2*>(smem_raw);     // {(y_x, y_x), (|y|^2, |y|^2)}
-    ulonglong2* sMid = sPt + kChunk;                               // {(ybar_x, ybar_x), (|ybar|^2, |ybar|^2)}
-    ulonglong2* sCr = sMid + kChunk;                               // {(dy_y/2, dy_y/2), (y_i x y_{i+1}, same)}
+    float4* sPM = reinterpret_cast<float4*>(smem_raw);             // (y_x, |y|^2, ybar_x, |ybar|^2)
+    float2* sCr = reinterpret_cast<float2*>(sPM + kChunk);         // (dy_y/2, y_i x y_{i+1})
 
     const int tid = threadIdx.x;
     const int tile = blockIdx.x % n_tiles;
@@ -76,7 +76,7 @@ k_wilson_sech2_f32(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit)
         float R2[P], ax[P], Tt[P];
 #pragma unroll
         for (int j = 0; j < P; ++j) {
-            gp[j] = tile * (kThreads * P) + j * kThreads + tid;
+            gp[j] = tile * (THREADS * P) + j * THREADS + tid;
             const int g = min(gp[j], n_grid - 1);
             const double T = a.T[g / a.n_rho];
             const double rho = a.rho[g % a.n_rho];
@@ -114,7 +114,7 @@ k_wilson_sech2_f32(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit)
         for (int c0 = 0; c0 < N; c0 += kChunk) {
             const int cn = min(kChunk, N - c0);
             __syncthreads();                                  // the previous chunk has been consumed
-            for (int i = tid; i < cn; i += kThreads) {        // stage: derived unit-loop quantities, FP64 -> FP32
+            for (int i = tid; i < cn; i += THREADS) {         // stage: derived unit-loop quantities, FP64 -> FP32
                 const int n = c0 + i;
                 const int n1 = (n + 1 == N) ? 0 : n + 1;      // closed loop, i+1 mod N
                 double yx, yy, zx, zy;
@@ -129,9 +129,8 @@ k_wilson_sech2_f32(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit)
                 const float f_yx = float(yx), f_y2 = float(yx * yx + yy * yy);
                 const float f_mx = float(mx), f_m2 = float(mx * mx + my * my);
                 const float f_hdy = float(0.5 * (zy - yy)), f_cr = float(yx * zy - yy * zx);
-                sPt[i] = make_ulonglong2(pk(f_yx, f_yx), pk(f_y2, f_y2));
-                sMid[i] = make_ulonglong2(pk(f_mx, f_mx), pk(f_m2, f_m2));
-                sCr[i] = make_ulonglong2(pk(f_hdy, f_hdy), pk(f_cr, f_cr));
+                sPM[i] = make_float4(f_yx, f_y2, f_mx, f_m2);
+                sCr[i] = make_float2(f_hdy, f_cr);
             }
             __syncthreads();
 
@@ -142,9 +141,13 @@ k_wilson_sech2_f32(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit)
                 const int ie = min(i0 + SUMBLOCK, cn);
 #pragma unroll UNROLL
                 for (int i = i0; i < ie; ++i) {
-                    const ulonglong2 pt = sPt[i];
-                    const ulonglong2 md = sMid[i];
-                    const ulonglong2 cx = sCr[i];
+                    // one LDS.128 + one LDS.64 per staged point (a broadcast: every lane reads the same address);
+                    // each scalar feeds FFMA2 as a both-halves operand (SASS: Rn.F32), no duplication in memory
+                    const float4 pm = sPM[i];
+                    const float2 cs = sCr[i];
+                    const ulonglong2 pt = make_ulonglong2(pk(pm.x, pm.x), pk(pm.y, pm.y));
+                    const ulonglong2 md = make_ulonglong2(pk(pm.z, pm.z), pk(pm.w, pm.w));
+                    const ulonglong2 cx = make_ulonglong2(pk(cs.x, cs.x), pk(cs.y, cs.y));
 #pragma unroll
                     for (int q = 0; q < Q; ++q) {
                         // |x_i|^2 and |m_i|^2 (times k^2): eq. (8), (25)-(28)
@@ -239,13 +242,15 @@ k_wilson_sech2_f32(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit)
 // plan.P grid points per thread; P = 1 (tiny grids) runs as a half-empty pair.
 cudaError_t launch_wilson_sech2_f32(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s)
 {
-    const size_t smem = 3 * sizeof(ulonglong2) * (size_t)kChunk;
+    const size_t smem = (sizeof(float4) + sizeof(float2)) * (size_t)kChunk;
     const int64_t n_ctas = plan.n_units * plan.n_tiles;
     if (n_ctas > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     const unsigned g = (unsigned)n_ctas;
     // LOGPOLY = true (5 special-function ops per point-eval), 4 CTAs/SM (64 registers), inner loop
     // unrolled by 2: the fastest of the combinations measured in profiles/r01_variants.md.
-#define WL_LAUNCH(PP) k_wilson_sech2_f32<PP, true, 4, 2, kSumBlock><<<g, kThreads, smem, s>>>(a, plan.n_grid, plan.n_tiles, plan.loops_per_unit)
+    // LOGPOLY = true (5 special-function ops per point-eval), 256 threads x P = 4, 4 CTAs/SM (64 registers),
+    // inner loop unrolled by 2: the fastest of the combinations measured (profiles/r01_variants.md).
+#define WL_LAUNCH(PP) k_wilson_sech2_f32<PP, kThreads, true, 4, 2, kSumBlock><<<g, kThreads, smem, s>>>(a, plan.n_grid, plan.n_tiles, plan.loops_per_unit)
     switch (plan.P) {
         case 2: WL_LAUNCH(2); break;
         case 4: WL_LAUNCH(4); break;
