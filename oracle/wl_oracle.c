@@ -284,6 +284,97 @@ void wlo_extrapolate(const double *lev3, int64_t n, double *W_inf, double *delta
 }
 
 /* ------------------------------------------------------------------------- */
+/* Effective-action integrals, eq. (12), (44)-(47), (70),     */
+/* 234-255, 417, 472, 495 (reading A16).                            */
+/*   density(rho) = int_0^inf dT e^{-m^2 T}/T^3 [ <W> - 1 - (eB_cm T)^2/3 ]    */
+/*   (scalar QED: [ <W> - 1 + (eB_cm T)^2/6 ], eq. (45))                       */
+/* = int_0^a of the small-T expansion (44)/(45), integrated term by term       */
+/* (eq. (47)), + int_a^inf by Simpson's rule in x = 1/(1 + T/Tmax)             */
+/* on n equal intervals of [0, x_a], x_a = 1/(1 + a/Tmax); the  */
+/* node x = 0 (T = inf) contributes nothing.  Done separately for every group  */
+/* of worldlines, so the error is the SEM of the group values.  */
+/* ------------------------------------------------------------------------- */
+
+/* Proper-time nodes T_j, j = 0..n-1, x_j = x_a (n - j)/n, T_j = Tmax (1/x_j - 1): T_0 = a, increasing. */
+int wlo_proper_time_nodes(double a, double Tmax, int n, double *T)
+{
+    if (!(a > 0.0) || !(Tmax > 0.0) || n < 2 || n % 2 != 0) return -1;
+    double xa = 1.0 / (1.0 + a / Tmax);
+    for (int j = 0; j < n; ++j) {
+        double x = xa * (double)(n - j) / (double)n;
+        T[j] = Tmax * (1.0 / x - 1.0);
+    }
+    T[0] = a;
+    return 0;
+}
+
+/* int_0^a of eq. (44) (fermion) or eq. (45) (scalar), b = eB(r_cm). */
+double wlo_small_T_integral(double b, double m2, double a, int scalar)
+{
+    double b4 = b * b * b * b, b6 = b4 * b * b;
+    double c1, c2, c3, c4;
+    if (!scalar) {                                  /* eq. (44) */
+        c1 = -b4 / 45.0;
+        c2 = b4 * m2 / 45.0;
+        c3 = 2.0 * b6 / 945.0 - b4 * m2 * m2 / 90.0;
+        c4 = (7.0 * b4 * m2 * m2 * m2 - 4.0 * b6 * m2) / 1890.0;
+    } else {                                        /* eq. (45) */
+        c1 = 7.0 * b4 / 360.0;
+        c2 = -7.0 * b4 * m2 / 360.0;
+        c3 = (147.0 * b4 * m2 * m2 - 31.0 * b6) / 15120.0;
+        c4 = (31.0 * b6 * m2 - 49.0 * b4 * m2 * m2 * m2) / 15120.0;
+    }
+    return c1 * a * a / 2.0 + c2 * a * a * a / 3.0 + c3 * a * a * a * a / 4.0 + c4 * a * a * a * a * a / 5.0;
+}
+
+/* group_sums [G][n_T][n_rho] at the nodes of wlo_proper_time_nodes(a, Tmax, n_T); density [G][n_rho]. */
+int wlo_action_density(int profile, const double *params, int scalar,
+                       const double *group_sums, int n_groups, int64_t n_loops,
+                       const double *T, int n_T, const double *rho_cm, int n_rho,
+                       double m2, double a, double Tmax, double *density)
+{
+    if (n_groups < 1 || n_loops < 1 || n_loops % n_groups != 0 || n_T < 2 || n_T % 2 != 0 || n_rho < 1) return -1;
+    if (!(a > 0.0) || !(Tmax > 0.0)) return -1;
+    const double per_group = (double)(n_loops / n_groups);
+    const double xa = 1.0 / (1.0 + a / Tmax);
+    const double h = xa / (double)n_T;
+    for (int g = 0; g < n_groups; ++g)
+        for (int r = 0; r < n_rho; ++r) {
+            double b = wlo_field_b(profile, params, rho_cm[r]);
+            double simpson = 0.0;
+            for (int j = 0; j < n_T; ++j) {
+                int k = n_T - j;                                     /* Simpson node index, x_k = k h */
+                double x = h * (double)k;
+                double Tj = T[j];
+                double W = group_sums[((int64_t)g * n_T + j) * n_rho + r] / per_group;     /* <W>_g, eq. (60) */
+                double bT = b * Tj;
+                double bracket = scalar ? W - 1.0 + bT * bT / 6.0 : W - 1.0 - bT * bT / 3.0;
+                double I = exp(-m2 * Tj) / (Tj * Tj * Tj) * bracket;                       /* eq. (70) */
+                double weight = (k == n_T) ? 1.0 : ((k % 2) ? 4.0 : 2.0);
+                simpson += weight * I * Tmax / (x * x);                                    /* dT = Tmax dx/x^2 */
+            }
+            density[(int64_t)g * n_rho + r] = wlo_small_T_integral(b, m2, a, scalar) + simpson * h / 3.0;
+        }
+    return 0;
+}
+
+/* eq. (12): action[g] = (1/4 pi) int rho density_g(rho) d rho by Simpson on a uniform rho grid (n_rho odd). */
+int wlo_action_radial(const double *density, int n_groups, const double *rho_cm, int n_rho, double *action)
+{
+    if (n_groups < 1 || n_rho < 3 || n_rho % 2 != 1) return -1;
+    const double h = (rho_cm[n_rho - 1] - rho_cm[0]) / (double)(n_rho - 1);
+    for (int g = 0; g < n_groups; ++g) {
+        double s = 0.0;
+        for (int r = 0; r < n_rho; ++r) {
+            double weight = (r == 0 || r == n_rho - 1) ? 1.0 : ((r % 2) ? 4.0 : 2.0);
+            s += weight * rho_cm[r] * density[(int64_t)g * n_rho + r];
+        }
+        action[g] = s * h / 3.0 / (4.0 * M_PI);
+    }
+    return 0;
+}
+
+/* ------------------------------------------------------------------------- */
 /* Jackknife finalise, eq. (60)-(63); delete-one-group means (reading A7).    */
 /*   mean, err [n_grid]; delete_one nullable [G][n_grid]                      */
 /* ------------------------------------------------------------------------- */

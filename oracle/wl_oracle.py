@@ -43,6 +43,15 @@ def lib():
                                               _dp, C.c_int, C.c_int, _dp, _dp]
         L.wlo_extrapolate.restype = None
         L.wlo_extrapolate.argtypes = [_dp, C.c_int64, _dp, _dp]
+        L.wlo_proper_time_nodes.restype = C.c_int
+        L.wlo_proper_time_nodes.argtypes = [C.c_double, C.c_double, C.c_int, _dp]
+        L.wlo_small_T_integral.restype = C.c_double
+        L.wlo_small_T_integral.argtypes = [C.c_double, C.c_double, C.c_double, C.c_int]
+        L.wlo_action_density.restype = C.c_int
+        L.wlo_action_density.argtypes = [C.c_int, _dp, C.c_int, _dp, C.c_int, C.c_int64, _dp, C.c_int, _dp, C.c_int,
+                                         C.c_double, C.c_double, C.c_double, _dp]
+        L.wlo_action_radial.restype = C.c_int
+        L.wlo_action_radial.argtypes = [_dp, C.c_int, _dp, C.c_int, _dp]
         L.wlo_finalize.restype = C.c_int
         L.wlo_finalize.argtypes = [_dp, C.c_int, C.c_int64, C.c_int64, _dp, _dp, _dp]
         L.wlo_philox4x32_10.restype = None
@@ -149,6 +158,45 @@ def extrapolate(levels):
     delta = np.empty(n)
     lib().wlo_extrapolate(_p(a), n, _p(out), _p(delta))
     return out.reshape(a.shape[1:]), delta.reshape(a.shape[1:])
+
+
+def proper_time_nodes(a, Tmax, n):
+    """Simpson nodes of x = 1/(1 + T/Tmax) on [0, x_a] as proper times T_0 = a < T_1 < ...."""
+    T = np.empty(n)
+    if lib().wlo_proper_time_nodes(float(a), float(Tmax), int(n), _p(T)) != 0:
+        raise ValueError("proper_time_nodes: a > 0, Tmax > 0, n even >= 2")
+    return T
+
+
+def small_T_integral(eB, m2, a, scalar=False):
+    """int_0^a of the small-T expansion eq. (44) (fermion) / (45) (scalar)."""
+    return lib().wlo_small_T_integral(float(eB), float(m2), float(a), 1 if scalar else 0)
+
+
+def action_density(profile, params, group_sums, n_loops, T, rho_cm, m2, a, Tmax, scalar=False):
+    """Per-group proper-time integral of eq. (12)/(70): density [G][n_rho] (eq. (47))."""
+    pr = _f64(params)
+    gs = _f64(group_sums)
+    T = _f64(T)
+    rho = _f64(rho_cm)
+    G = gs.shape[0]
+    assert gs.shape == (G, T.shape[0], rho.shape[0])
+    out = np.empty((G, rho.shape[0]))
+    rc = lib().wlo_action_density(profile, _p(pr), 1 if scalar else 0, _p(gs), G, int(n_loops), _p(T), T.shape[0],
+                                  _p(rho), rho.shape[0], float(m2), float(a), float(Tmax), _p(out))
+    if rc != 0:
+        raise ValueError("wlo_action_density: invalid argument")
+    return out
+
+
+def action_radial(density, rho_cm):
+    """eq. (12): (1/4 pi) int rho density d rho per group, Simpson on a uniform grid (n_rho odd)."""
+    d = _f64(density)
+    rho = _f64(rho_cm)
+    out = np.empty(d.shape[0])
+    if lib().wlo_action_radial(_p(d), d.shape[0], _p(rho), rho.shape[0], _p(out)) != 0:
+        raise ValueError("wlo_action_radial: n_rho must be odd >= 3")
+    return out
 
 
 def finalize(group_sums, n_loops, delete_one=False):
