@@ -169,6 +169,30 @@ wl_status wl_eval_discretization(const wl_field* field,
  *   d_W_inf[k] = 8/3 W_N - 2 W_{N/2} + 1/3 W_{N/4},   d_delta[k] = |W_N - W_inf|  (d_delta may be NULL). */
 wl_status wl_extrapolate(const double* d_levels3, int64_t n, double* d_W_inf, double* d_delta, void* stream);
 
+/* Effective-action integrals (eq. (12), (44)-(47), (70); DESIGN.md
+ * reading A16), done separately for every group of worldlines so that the error of the result is the
+ * standard error of the group values.
+ *
+ * wl_proper_time_nodes (host only): the n_T (even) proper times at which <W> must be evaluated, the
+ * Simpson nodes of x = 1/(1 + T/Tmax) on [0, x_a], x_a = 1/(1 + a/Tmax):
+ *   h_T[j] = Tmax (1/x_j - 1),  x_j = x_a (n_T - j)/n_T,  j = 0..n_T-1   (h_T[0] = a, increasing).
+ *
+ * wl_action_density: from d_group_sums[G][n_T][n_rho] (wl_eval at those nodes),
+ *   d_density[g][r] = int_0^a (small-T expansion eq. (44), or (45) for a scalar field)   [eq. (47)]
+ *                   + Simpson int_a^inf dT e^{-m2 T}/T^3 [ <W>_g - 1 - (eB(rho_r) T)^2/3 ]  [eq. (12), (70)]
+ *   (scalar field: [ <W>_g - 1 + (eB T)^2/6 ]), <W>_g = S_g G/n_loops, eB(rho) from the field profile.
+ *   m2 = m^2 >= 0, a > 0, Tmax > 0, n_T even >= 2, n_loops % G == 0; else WL_ERR_INVALID_ARG.
+ *   wl_jackknife_finalize(d_density, G, G, 1, n_rho, ...) then gives its mean and error over the groups.
+ *
+ * wl_action_radial: d_action[g] = (1/4 pi) int rho d_density[g](rho) d rho by Simpson's rule on the uniform
+ *   grid d_rho_cm (n_rho odd >= 3, else WL_ERR_INVALID_ARG): Gamma/(T L_z) of eq. (12) per group. */
+wl_status wl_proper_time_nodes(double a, double Tmax, int n_T, double* h_T);
+wl_status wl_action_density(const wl_field* field, const double* d_group_sums, int n_groups, int64_t n_loops,
+                            const double* d_T, int n_T, const double* d_rho_cm, int n_rho,
+                            double m2, double a, double Tmax, double* d_density, void* stream);
+wl_status wl_action_radial(const double* d_density, int n_groups, const double* d_rho_cm, int n_rho,
+                           double* d_action, void* stream);
+
 /* Jackknife finalise, eq. (60)-(63).  From d_group_sums[G][n_T][n_rho]:
  *   d_mean[t][r] = (sum_g S_g)/n_loops,
  *   d_err[t][r]  = sqrt(sum_g (S_g G/n_loops - mean)^2 / (G (G-1))),

@@ -53,6 +53,13 @@ _lib.wl_eval_discretization.argtypes = [_vp, _vp, _int, _i64, _int, _dp, _int, _
                                         _vp, _sz, _vp]
 _lib.wl_extrapolate.restype = _int
 _lib.wl_extrapolate.argtypes = [_dp, _i64, _dp, _dp, _vp]
+_lib.wl_proper_time_nodes.restype = _int
+_lib.wl_proper_time_nodes.argtypes = [C.c_double, C.c_double, _int, C.POINTER(C.c_double)]
+_lib.wl_action_density.restype = _int
+_lib.wl_action_density.argtypes = [_vp, _dp, _int, _i64, _dp, _int, _dp, _int, C.c_double, C.c_double, C.c_double,
+                                   _dp, _vp]
+_lib.wl_action_radial.restype = _int
+_lib.wl_action_radial.argtypes = [_dp, _int, _dp, _int, _dp, _vp]
 _lib.wl_eval_per_loop.restype = _int
 _lib.wl_eval_per_loop.argtypes = [_vp, _vp, _int, _i64, _int, _dp, _int, _dp, _dp, _int, _int, _dp, _dp,
                                   _dp, _vp]
@@ -314,3 +321,38 @@ def wl_eval_host(field, loops, T, rho_cm, phi_cm=None, n_groups=2, compute=torch
 def wl_eval_host_trim():
     """Returns the unused memory of wl_eval_host's private pool to the device."""
     _check(_lib.wl_eval_host_trim(), "wl_eval_host_trim")
+
+
+def wl_proper_time_nodes(a, Tmax, n_T) -> np.ndarray:
+    """Host: the n_T proper times (Simpson nodes of x = 1/(1+T/Tmax)), increasing from a."""
+    T = np.empty(int(n_T), dtype=np.float64)
+    _check(_lib.wl_proper_time_nodes(float(a), float(Tmax), int(n_T), T.ctypes.data_as(C.POINTER(C.c_double))),
+           "wl_proper_time_nodes")
+    return T
+
+
+def wl_action_density(field, group_sums, n_loops, T, rho_cm, m2, a, Tmax, stream=None):
+    """Per-group proper-time integral of eq. (12)/(70): density [G][n_rho]; see include/wl.h."""
+    gs = _cuda_f64(group_sums, "group_sums")
+    T = _cuda_f64(T, "T")
+    rho_cm = _cuda_f64(rho_cm, "rho_cm")
+    G, n_T, n_rho = gs.shape
+    if T.numel() != n_T or rho_cm.numel() != n_rho:
+        raise ValueError("group_sums must be [G][n_T][n_rho]")
+    out = torch.empty((G, n_rho), dtype=torch.float64, device=gs.device)
+    with torch.cuda.device(gs.device):
+        _check(_lib.wl_action_density(field._h, _ptr(gs), G, int(n_loops), _ptr(T), n_T, _ptr(rho_cm), n_rho,
+                                      float(m2), float(a), float(Tmax), _ptr(out), _stream(stream)),
+               "wl_action_density")
+    return out
+
+
+def wl_action_radial(density, rho_cm, stream=None):
+    """(1/4 pi) int rho density d rho per group (eq. (12)), Simpson on the uniform grid rho_cm (n_rho odd)."""
+    d = _cuda_f64(density, "density")
+    rho_cm = _cuda_f64(rho_cm, "rho_cm", d.shape[1])
+    out = torch.empty((d.shape[0],), dtype=torch.float64, device=d.device)
+    with torch.cuda.device(d.device):
+        _check(_lib.wl_action_radial(_ptr(d), d.shape[0], _ptr(rho_cm), d.shape[1], _ptr(out), _stream(stream)),
+               "wl_action_radial")
+    return out

@@ -113,3 +113,17 @@ def test_compute_calls_reject_bad_arguments_without_a_gpu(lib):
     lib.wl_jackknife_finalize.argtypes = [vp, C.c_int, C.c_int64, C.c_int, C.c_int, vp, vp, vp, vp]
     assert lib.wl_jackknife_finalize(dummy, 1, 8, 2, 2, dummy, dummy, None, None) == 1   # G < 2
     assert lib.wl_jackknife_finalize(dummy, 3, 8, 2, 2, dummy, dummy, None, None) == 1   # 8 % 3
+
+
+def test_proper_time_nodes_host_call(lib):
+    """wl_proper_time_nodes is host-only: x = 1/(1 + T/Tmax) is uniform on (0, x_a]."""
+    lib.wl_proper_time_nodes.restype = C.c_int
+    lib.wl_proper_time_nodes.argtypes = [C.c_double, C.c_double, C.c_int, C.POINTER(C.c_double)]
+    n, a, Tmax = 12, 0.05, 3.0
+    T = (C.c_double * n)()
+    assert lib.wl_proper_time_nodes(a, Tmax, n, T) == 0
+    x = [1.0 / (1.0 + t / Tmax) for t in T]
+    xa = 1.0 / (1.0 + a / Tmax)
+    assert T[0] == a and all(abs(x[j] - xa * (n - j) / n) < 1e-15 for j in range(n))
+    assert lib.wl_proper_time_nodes(a, Tmax, 7, T) == 1 and lib.wl_proper_time_nodes(0.0, Tmax, 8, T) == 1
+    assert lib.wl_proper_time_nodes(a, Tmax, 8, None) == 1
