@@ -17,18 +17,24 @@ __device__ __forceinline__ void unpack(u64 v, float& a, float& b) { asm("mov.b64
 __device__ __forceinline__ u64 ffma2(u64 a, u64 b, u64 c) { u64 r; asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
 #define MUFU(op, x) asm volatile(op ".approx.ftz.f32 %0, %0;" : "+f"(x))
 
-enum { FFMA3 = 0, FFMA2X, EX2, RSQRT, SQRT, LG2, DFMA, F2F_DADD, MIX_SCALAR, MIX_PACKED };
+enum { FFMA3 = 0, FFMA2X, FFMA2_2VAR, FFMA2_3VAR, EX2, RSQRT, SQRT, LG2, DFMA, F2F_DADD, MIX_SCALAR, MIX_PACKED, MIX_LDS };
 
 // One loop iteration issues, per warp:
 //   FFMA3: 32 three-register FFMA      FFMA2X: 16 FFMA2 (= 32 FMAs)      EX2..LG2: 32 MUFU
 //   DFMA: 32 DFMA                      F2F_DADD: 4 x (F2F.F64.F32 + DADD)
 //   MIX_SCALAR: M MUFU.EX2 + F FFMA    MIX_PACKED: M MUFU.EX2 + F FFMA2 + A FMNMX
+//   FFMA2_2VAR / FFMA2_3VAR: 16 FFMA2 whose sources are two / three different, changing register pairs
+//   MIX_LDS: M MUFU.EX2 + F FFMA2 + A broadcast LDS.128 (every lane reads the same address)
 template <int KIND, int M, int F, int A>
 __global__ void k(float* out, int iters, float s1, float s2)
 {
+    __shared__ float4 sm[256];
+    sm[threadIdx.x] = make_float4(s1, s2, s1, s2);
+    __syncthreads();
     float a[8];
     u64 p[4];
     double d[4];
+    float lds_acc = 0.0f;
     float b = s1 + threadIdx.x * 1e-9f, c = s2;
     const u64 bb = pack(b, b), cc = pack(c, c);
 #pragma unroll
@@ -42,6 +48,12 @@ __global__ void k(float* out, int iters, float s1, float s2)
         } else if (KIND == FFMA2X) {
 #pragma unroll
             for (int r = 0; r < 16; ++r) p[r & 3] = ffma2(p[r & 3], bb, cc);
+        } else if (KIND == FFMA2_2VAR) {
+#pragma unroll
+            for (int r = 0; r < 16; ++r) p[r & 3] = ffma2(p[r & 3], p[(r + 1) & 3], cc);
+        } else if (KIND == FFMA2_3VAR) {
+#pragma unroll
+            for (int r = 0; r < 16; ++r) p[r & 3] = ffma2(p[r & 3], p[(r + 1) & 3], p[(r + 2) & 3]);
         } else if (KIND == EX2) {
 #pragma unroll
             for (int r = 0; r < 32; ++r) MUFU("ex2", a[r & 7]);
@@ -76,9 +88,23 @@ __global__ void k(float* out, int iters, float s1, float s2)
             }
 #pragma unroll
             for (int x = 0; x < A; ++x) a[7 - (x & 1)] = fmaxf(a[7 - (x & 1)], b);
+        } else if (KIND == MIX_LDS) {
+#pragma unroll
+            for (int m = 0; m < M; ++m) {
+                MUFU("ex2", a[m & 7]);
+#pragma unroll
+                for (int f = 0; f < F / M; ++f) { const int q = (m + f) & 3; p[q] = ffma2(p[q], bb, cc); }
+            }
+#pragma unroll
+            for (int x = 0; x < A; ++x) {
+                float4 v;
+                const unsigned addr = (unsigned)__cvta_generic_to_shared(&sm[(it * A + x) & 255]);
+                asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+                lds_acc += v.x;
+            }
         }
     }
-    float s = c;
+    float s = c + lds_acc;
     for (int i = 0; i < 8; ++i) s += a[i];
     for (int i = 0; i < 4; ++i) { float x, y; unpack(p[i], x, y); s += x + y + (float)d[i]; }
     out[blockIdx.x * blockDim.x + threadIdx.x] = s;
@@ -120,6 +146,8 @@ int main()
     printf("| test (per warp per loop iteration) | ms | clk / iter / sub-partition | lanes / clk / SM | note |\n|---|---|---|---|---|\n");
     run<FFMA3, 0, 0, 0>("32 FFMA (3 registers)", 32, "FP32 FMA pipe, scalar");
     run<FFMA2X, 0, 0, 0>("16 FFMA2 (= 32 FMAs)", 32, "packed: same FMA rate, half the issue slots");
+    run<FFMA2_2VAR, 0, 0, 0>("16 FFMA2, 2 varying source pairs", 32, "register reads start to cost");
+    run<FFMA2_3VAR, 0, 0, 0>("16 FFMA2, 3 varying source pairs", 32, "six registers per lane: 3 clk per FFMA2");
     run<EX2, 0, 0, 0>("32 MUFU.EX2", 32, "XU pipe");
     run<RSQRT, 0, 0, 0>("32 MUFU.RSQ", 32, "XU pipe");
     run<SQRT, 0, 0, 0>("32 MUFU.SQRT", 32, "XU pipe");
@@ -137,5 +165,9 @@ int main()
     run<MIX_PACKED, 5, 20, 0>("5 MUFU + 20 FFMA2 (40 FMAs)", 0, "XU bound = 40, FMA pipe 40");
     run<MIX_PACKED, 5, 15, 6>("5 MUFU + 15 FFMA2 + 6 FMNMX", 0, "ALU-pipe work is nearly free");
     run<MIX_PACKED, 4, 16, 0>("4 MUFU + 16 FFMA2 (32 FMAs)", 0, "XU bound = 32, FMA pipe 32");
+    run<MIX_LDS, 5, 15, 1>("5 MUFU + 15 FFMA2 + 1 LDS.128", 0, "shared-memory loads return through the XU's queue");
+    run<MIX_LDS, 5, 15, 2>("5 MUFU + 15 FFMA2 + 2 LDS.128", 0, "");
+    run<MIX_LDS, 5, 15, 4>("5 MUFU + 15 FFMA2 + 4 LDS.128", 0, "about 4 clk per LDS.128");
+    run<MIX_LDS, 5, 15, 8>("5 MUFU + 15 FFMA2 + 8 LDS.128", 0, "");
     return 0;
 }
