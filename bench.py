@@ -353,8 +353,10 @@ def run_ours(args, cfg):
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_wilson launch from the `ncu --set full` capture
 # summarised under profiles/ (per launch, like `achieved`); None until measured for that workload.
 NCU_TRAFFIC_BYTES = {
-    # profiles/r01_wilson_f32_ncu.md: 279.2 MB read (the 268.4 MB ensemble once) + 58.8 MB written (partials)
-    ("cfg3_paper_scale", "f32"): 279201280 + 58751232,
+    # profiles/r01_wilson_f32_ncu.md: 279.8 MB read (the 268.4 MB ensemble once) + 58.4 MB written (partials)
+    ("cfg3_paper_scale", "f32"): 279834624 + 58382848,
+    # profiles/r01_wilson_f64_ncu.md: 4.2 MB read, partials still in L2
+    ("cfg1_small_sech2", "f64"): 4216832,
 }
 
 
