@@ -44,52 +44,43 @@ __device__ __forceinline__ void sqrt_rsqrt(double w, double& s, double& ir)
     ir = h + h;
 }
 
-// 2^(-u) for u >= 0.  u = n + f, n = rint(u), |f| <= 1/2; 2^(-f) by a degree-10 polynomial (rel. error
-// 3e-16); 2^(-n) by subtracting n from the exponent field (n clamped to 1000: the result is then < 1e-301).
+// Polynomial coefficients live in constant memory: a DFMA takes one constant-bank operand directly, whereas
+// a 64-bit literal costs two uniform-register moves per use (74 extra instructions per two point-evals).
+__constant__ double kExp2[11] = {   // 2^(-f), |f| <= 1/2: gen_h_poly.py E2 10 (rel. error 3e-16), highest degree first
+    7.0725859492692236999e-9, -1.0208690299958305835e-7, 1.3215442587921689653e-6, -0.000015252657260200837064,
+    0.00015403530441736050155, -0.0013333558230164973899, 0.0096181291076068885273, -0.055504108664447719166,
+    0.2402265069591009822, -0.69314718055994998286, 1.0};
+__constant__ double kLog[21] = {    // 1 - log2(1+E), E in [0,1]: gen_h_poly.py L 20 (abs. error 2e-17), highest degree first
+    0.000037716935465554877791, -0.00043656761569165172581, 0.0024001133617501894281, -0.0083829321823817315509,
+    0.021049247229017102326, -0.040925999935882766517, 0.065142917694358537062, -0.089143555615740867799,
+    0.10983761672477964967, -0.12712681926472003036, 0.14301332675890233011, -0.15998872460281850448,
+    0.1802769786868982234, -0.20609048918280538869, 0.24044821605097346373, -0.28853893413338524963,
+    0.360673756378019119, -0.4808983468401831136, 0.72134752044239441043, -1.4426950408889492514,
+    0.99999999999999998397};
+__constant__ double kHPoly[8] = {   // h(w)/(4 log2 e) in w', w = u^2 < 1/16: gen_h_poly.py hs 0.0625 7, highest degree first
+    -7.7102839224224163556e-11, 1.7289132522207449606e-9, -3.519550981355539808e-8, 7.0992077974390822073e-7,
+    -0.000014180275863490838682, 0.00027778246137776088779, -0.0052035101873268705174, 0.086643397569993163057};
+
+// 2^(-u) for u >= 0.  u = n + f, n = rint(u), |f| <= 1/2; 2^(-f) by a degree-10 polynomial; 2^(-n) by
+// subtracting n from the exponent field (n clamped to 1000: the result is then < 1e-301).
 __device__ __forceinline__ double exp2_neg(double u)
 {
     const double kMagic = 6755399441055744.0;            // 1.5 * 2^52
     const double t = u + kMagic;
     const double f = u - (t - kMagic);
-    double p = 7.0725859492692236999e-9;
-    p = fma(p, f, -1.0208690299958305835e-7);
-    p = fma(p, f, 1.3215442587921689653e-6);
-    p = fma(p, f, -0.000015252657260200837064);
-    p = fma(p, f, 0.00015403530441736050155);
-    p = fma(p, f, -0.0013333558230164973899);
-    p = fma(p, f, 0.0096181291076068885273);
-    p = fma(p, f, -0.055504108664447719166);
-    p = fma(p, f, 0.2402265069591009822);
-    p = fma(p, f, -0.69314718055994998286);
-    p = fma(p, f, 1.0);
+    double p = kExp2[0];
+#pragma unroll
+    for (int i = 1; i < 11; ++i) p = fma(p, f, kExp2[i]);
     const int n = min(__double2loint(t), 1000);
     return __hiloint2double(__double2hiint(p) - (n << 20), __double2loint(p));
 }
 
-// 1 - log2(1+E), E in [0,1]: degree-20 polynomial (abs. error 2e-17 + rounding).
+// 1 - log2(1+E), E in [0,1]: degree-20 polynomial.
 __device__ __forceinline__ double one_minus_log2_1p(double E)
 {
-    double L = 0.000037716935465554877791;
-    L = fma(L, E, -0.00043656761569165172581);
-    L = fma(L, E, 0.0024001133617501894281);
-    L = fma(L, E, -0.0083829321823817315509);
-    L = fma(L, E, 0.021049247229017102326);
-    L = fma(L, E, -0.040925999935882766517);
-    L = fma(L, E, 0.065142917694358537062);
-    L = fma(L, E, -0.089143555615740867799);
-    L = fma(L, E, 0.10983761672477964967);
-    L = fma(L, E, -0.12712681926472003036);
-    L = fma(L, E, 0.14301332675890233011);
-    L = fma(L, E, -0.15998872460281850448);
-    L = fma(L, E, 0.1802769786868982234);
-    L = fma(L, E, -0.20609048918280538869);
-    L = fma(L, E, 0.24044821605097346373);
-    L = fma(L, E, -0.28853893413338524963);
-    L = fma(L, E, 0.360673756378019119);
-    L = fma(L, E, -0.4808983468401831136);
-    L = fma(L, E, 0.72134752044239441043);
-    L = fma(L, E, -1.4426950408889492514);
-    L = fma(L, E, 0.99999999999999998397);
+    double L = kLog[0];
+#pragma unroll
+    for (int i = 1; i < 21; ++i) L = fma(L, E, kLog[i]);
     return L;
 }
 
@@ -186,14 +177,9 @@ k_wilson_sech2_f64(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit)
                     const double br = fma(-um, Em * im, one_minus_log2_1p(Em));   // (1 - log2(1+E_m)) - u' E_m/(1+E_m)
                     const double hE = br * (irm * irm);                       // br / w'
                     // h(w)/(4 log2 e) in w', w = u^2 < 1/16 (gen_h_poly.py hs 0.0625 7)
-                    double hP = -7.7102839224224163556e-11;
-                    hP = fma(hP, wm, 1.7289132522207449606e-9);
-                    hP = fma(hP, wm, -3.519550981355539808e-8);
-                    hP = fma(hP, wm, 7.0992077974390822073e-7);
-                    hP = fma(hP, wm, -0.000014180275863490838682);
-                    hP = fma(hP, wm, 0.00027778246137776088779);
-                    hP = fma(hP, wm, -0.0052035101873268705174);
-                    hP = fma(hP, wm, 0.086643397569993163057);
+                    double hP = kHPoly[0];
+#pragma unroll
+                    for (int i = 1; i < 8; ++i) hP = fma(hP, wm, kHPoly[i]);
                     const double gt = (wm < kPolyBelow) ? hP : hE;
                     const double cr = fma(ax[j], cx.x, Tt[j] * cx.y);         // k^2 (m x d), eq. (24)
                     ph[j] = fma(gt, cr, ph[j]);
