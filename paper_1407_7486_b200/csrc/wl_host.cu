@@ -1,5 +1,7 @@
 // wl_host.cu -- wl_eval_host: the end-to-end call on HOST buffers (include/wl.h).
 // The only entry point that allocates device memory, copies and synchronises.
+#include <mutex>
+
 #include "wl_internal.cuh"
 
 namespace {
@@ -8,9 +10,11 @@ namespace {
 // what it has been given between calls (release threshold = max), so that a second call of the
 // same size pays no cudaMalloc/cudaFree; wl_eval_host_trim() gives the memory back.
 cudaMemPool_t g_pool[64] = {};
+std::mutex g_pool_mutex;
 
 cudaError_t host_pool(cudaMemPool_t* out)
 {
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
@@ -53,6 +57,7 @@ struct DeviceBuffers {
 
 extern "C" wl_status wl_eval_host_trim(void)
 {
+    std::lock_guard<std::mutex> lock(g_pool_mutex);
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return WL_ERR_CUDA; }
     if (dev >= 0 && dev < 64 && g_pool[dev]) {
