@@ -288,14 +288,16 @@ static cudaError_t launch_r(const EvalPlan& plan, const EvalArgs& a, int profile
 
 cudaError_t launch_wilson(const EvalPlan& plan, const EvalArgs& a, int profile, wl_dtype compute, cudaStream_t s)
 {
-    if (a.disc)
-        return compute == WL_F32 ? launch_r<float>(plan, a, profile, s) : launch_r<double>(plan, a, profile, s);
     // The lean sech^2 kernels carry squared radii scaled by (2 log2(e)/lambda)^2; outside this range of
     // lambda the FP32 one could overflow or flush, so the generic kernel (unscaled) serves it.
     const bool lambda_ok = a.p1 >= 1e-4 && a.p1 <= 1e4;
     if (compute == WL_F32 && profile == WL_PROFILE_SECH2 && a.phi == nullptr && lambda_ok) {
         EvalPlan p2 = plan;                              // grid points go in register pairs there
         if (p2.P < 2) { p2.P = 2; p2.n_tiles = (p2.n_grid + kThreads * 2 - 1) / (kThreads * 2); }
+        if (a.disc && p2.P == 2 && p2.n_grid >= kThreads * 8) {   // the discretisation plan caps P at 2 for the generic kernel
+            p2.P = 4;
+            p2.n_tiles = (p2.n_grid + kThreads * 4 - 1) / (kThreads * 4);
+        }
         return launch_wilson_sech2_f32(p2, a, s);
     }
     if (compute == WL_F64 && profile == WL_PROFILE_SECH2 && a.phi == nullptr)

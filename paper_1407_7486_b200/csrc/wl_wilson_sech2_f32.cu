@@ -51,9 +51,11 @@ __device__ __forceinline__ float xu_lg2_abs(float x) { float y; asm("lg2.approx.
 
 }  // namespace
 
-template <int P, int THREADS, bool LOGPOLY, int MINB, int UNROLL, int SUMBLOCK>
+// DISC = true: the discretisation estimate (eq. (48)-(50)); the two passes, the three levels and the
+// partial-sum layout are those of k_wilson<..., DISC = true> in wl_eval_kernels.cu.
+template <int P, int THREADS, bool LOGPOLY, int MINB, int UNROLL, int SUMBLOCK, bool DISC>
 __global__ void __launch_bounds__(THREADS, MINB)
-k_wilson_sech2_f32(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit)
+k_wilson_sech2_f32(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit, int64_t n_units)
 {
     static_assert(P % 2 == 0, "grid points are processed as register pairs");
     constexpr int Q = P / 2;
@@ -99,9 +101,12 @@ k_wilson_sech2_f32(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit)
               h2 = pk(0.000277586359849f, 0.000277586359849f), h3 = pk(-1.39101401155e-5f, -1.39101401155e-5f),
               h4 = pk(5.53576426559e-7f, 5.53576426559e-7f);
 
-    double Wsum[P];
+    constexpr int kLevels = DISC ? 3 : 1;
+    double Wsum[kLevels][P];
 #pragma unroll
-    for (int j = 0; j < P; ++j) Wsum[j] = 0.0;
+    for (int v = 0; v < kLevels; ++v)
+#pragma unroll
+        for (int j = 0; j < P; ++j) Wsum[v][j] = 0.0;
 
     for (int ll = 0; ll < loops_per_unit; ++ll) {
         const int64_t loop = unit * loops_per_unit + ll;
@@ -110,13 +115,25 @@ k_wilson_sech2_f32(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit)
         double dph[P], dsp[P];
 #pragma unroll
         for (int j = 0; j < P; ++j) { dph[j] = 0.0; dsp[j] = 0.0; }
+        double S2[DISC ? P : 1], B2[DISC ? P : 1];       // pass-0 sums (DISC only)
 
-        for (int c0 = 0; c0 < N; c0 += kChunk) {
-            const int cn = min(kChunk, N - c0);
+      const int Nv = DISC ? N / 2 : N;                  // terms per pass
+      for (int pass = 0; pass < (DISC ? 2 : 1); ++pass) {
+        if (DISC && pass == 1) {
+#pragma unroll
+            for (int j = 0; j < P; ++j) { S2[j] = dph[j]; B2[j] = dsp[j]; dph[j] = 0.0; dsp[j] = 0.0; }
+        }
+        for (int c0 = 0; c0 < Nv; c0 += kChunk) {
+            const int cn = min(kChunk, Nv - c0);
             __syncthreads();                                  // the previous chunk has been consumed
             for (int i = tid; i < cn; i += THREADS) {         // stage: derived unit-loop quantities, FP64 -> FP32
-                const int n = c0 + i;
-                const int n1 = (n + 1 == N) ? 0 : n + 1;      // closed loop, i+1 mod N
+                int n = c0 + i;
+                int n1 = (n + 1 == N) ? 0 : n + 1;            // closed loop, i+1 mod N
+                if (DISC) {                                   // sub-worldline: every 2nd / 4th point, closed on itself
+                    n = pass + 2 * (c0 + i);
+                    n1 = n + (pass ? 4 : 2);
+                    if (n1 >= N) n1 -= N;
+                }
                 double yx, yy, zx, zy;
                 if (a.loops_are_f64) {
                     const double2 u = L64[n], v = L64[n1];
@@ -217,6 +234,8 @@ k_wilson_sech2_f32(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit)
             }
         }
 
+      }   // pass
+
         // ---- W = cos(phase) cosh(spin), FP64, once per (loop, grid point): eq. (18), PAPER.md:121 ----
         const double g_scale = eB0 * lambda * lambda * 0.69314718055994530942;
         const double b_scale = 4.0 * eB0;
@@ -224,19 +243,30 @@ k_wilson_sech2_f32(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit)
         for (int j = 0; j < P; ++j) {
             const int g = min(gp[j], n_grid - 1);
             const double T = a.T[g / a.n_rho];
-            const double phase = g_scale * dph[j];
-            const double spin = b_scale * (T / double(N)) * dsp[j];
-            const double W = a.scalar ? cos(phase) : cos(phase) * cosh(spin);
-            Wsum[j] += W;
-            if (gp[j] < n_grid) {
-                if (a.phase_out) a.phase_out[loop * n_grid + gp[j]] = phase;
-                if (a.spin_out) a.spin_out[loop * n_grid + gp[j]] = spin;
+            if (!DISC) {
+                const double phase = g_scale * dph[j];
+                const double spin = b_scale * (T / double(N)) * dsp[j];
+                const double W = a.scalar ? cos(phase) : cos(phase) * cosh(spin);
+                Wsum[0][j] += W;
+                if (gp[j] < n_grid) {
+                    if (a.phase_out) a.phase_out[loop * n_grid + gp[j]] = phase;
+                    if (a.spin_out) a.spin_out[loop * n_grid + gp[j]] = spin;
+                }
+            } else {
+                const double S4 = dph[j], B4 = dsp[j], c = b_scale * (T / double(N));
+                const double phase[3] = {g_scale * (0.5 * S4), g_scale * S2[j], g_scale * (0.5 * S2[j] + 0.25 * S4)};   // eq. (48)-(50)
+                const double spin[3] = {2.0 * c * B4, 2.0 * c * B2[j], c * (B2[j] + B4)};
+#pragma unroll
+                for (int v = 0; v < 3; ++v)
+                    Wsum[v][j] += a.scalar ? cos(phase[v]) : cos(phase[v]) * cosh(spin[v]);
             }
         }
     }
 #pragma unroll
-    for (int j = 0; j < P; ++j)
-        if (gp[j] < n_grid) a.partial[unit * n_grid + gp[j]] = Wsum[j];
+    for (int v = 0; v < kLevels; ++v)
+#pragma unroll
+        for (int j = 0; j < P; ++j)
+            if (gp[j] < n_grid) a.partial[((int64_t)v * n_units + unit) * n_grid + gp[j]] = Wsum[v][j];
 }
 
 // plan.P grid points per thread; P = 1 (tiny grids) runs as a half-empty pair.
@@ -250,11 +280,19 @@ cudaError_t launch_wilson_sech2_f32(const EvalPlan& plan, const EvalArgs& a, cud
     // unrolled by 2: the fastest of the combinations measured in profiles/r01_variants.md.
     // LOGPOLY = true (5 special-function ops per point-eval), 256 threads x P = 4, 4 CTAs/SM (64 registers),
     // inner loop unrolled by 2: the fastest of the combinations measured (profiles/r01_variants.md).
-#define WL_LAUNCH(PP) k_wilson_sech2_f32<PP, kThreads, true, 4, 2, kSumBlock><<<g, kThreads, smem, s>>>(a, plan.n_grid, plan.n_tiles, plan.loops_per_unit)
-    switch (plan.P) {
-        case 2: WL_LAUNCH(2); break;
-        case 4: WL_LAUNCH(4); break;
-        default: return cudaErrorInvalidValue;
+#define WL_LAUNCH(PP, DD) k_wilson_sech2_f32<PP, kThreads, true, 4, 2, kSumBlock, DD><<<g, kThreads, smem, s>>>(a, plan.n_grid, plan.n_tiles, plan.loops_per_unit, plan.n_units)
+    if (a.disc) {
+        switch (plan.P) {
+            case 2: WL_LAUNCH(2, true); break;
+            case 4: WL_LAUNCH(4, true); break;
+            default: return cudaErrorInvalidValue;
+        }
+    } else {
+        switch (plan.P) {
+            case 2: WL_LAUNCH(2, false); break;
+            case 4: WL_LAUNCH(4, false); break;
+            default: return cudaErrorInvalidValue;
+        }
     }
 #undef WL_LAUNCH
     return cudaGetLastError();

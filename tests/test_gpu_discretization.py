@@ -63,6 +63,15 @@ def test_level_N_over_2_is_the_ordinary_run_on_every_other_point(api):
     _, gs = api.wl_eval(f, loops[:, 0::2].contiguous(), T, rho, None, n_groups=4, compute="f64")
     torch.cuda.synchronize()
     assert torch.equal(gs3[1], gs)
+    # the lean sech^2 kernels serve both calls too (FP32: 64 x 64 grid so that both run 4 grid points per thread)
+    fs = api.wl_field_create(inputs.SECH2, (1.0, 1.0))
+    c = inputs.config(3)
+    T3, rho3, _ = c.grids()
+    for compute in ("f64", "f32"):
+        gs3 = api.wl_eval_discretization(fs, loops, dev(T3), dev(rho3), None, n_groups=4, compute=compute)
+        _, gs = api.wl_eval(fs, loops[:, 0::2].contiguous(), dev(T3), dev(rho3), None, n_groups=4, compute=compute)
+        torch.cuda.synchronize()
+        assert torch.equal(gs3[1], gs)
 
 
 def test_extrapolation_and_error_estimate(api, o):
