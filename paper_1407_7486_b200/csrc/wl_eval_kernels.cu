@@ -300,6 +300,15 @@ cudaError_t launch_wilson(const EvalPlan& plan, const EvalArgs& a, int profile, 
         }
         return launch_wilson_sech2_f32(p2, a, s);
     }
+    if (compute == WL_F32 && profile == WL_PROFILE_FLUXTUBE && a.phi == nullptr && lambda_ok) {
+        EvalPlan p2 = plan;
+        if (p2.P < 2) { p2.P = 2; p2.n_tiles = (p2.n_grid + kThreads * 2 - 1) / (kThreads * 2); }
+        if (a.disc && p2.P == 2 && p2.n_grid >= kThreads * 8) {
+            p2.P = 4;
+            p2.n_tiles = (p2.n_grid + kThreads * 4 - 1) / (kThreads * 4);
+        }
+        return launch_wilson_fluxtube_f32(p2, a, s);
+    }
     if (compute == WL_F64 && profile == WL_PROFILE_SECH2 && a.phi == nullptr)
         return launch_wilson_sech2_f64(plan, a, s);
     return compute == WL_F32 ? launch_r<float>(plan, a, profile, s) : launch_r<double>(plan, a, profile, s);

@@ -54,6 +54,8 @@ cudaError_t launch_wilson(const EvalPlan& plan, const EvalArgs& a, int profile, 
                           cudaStream_t s);
 // FP32, sech^2, phi_cm == NULL: the packed-FP32 kernel of wl_wilson_sech2_f32.cu (plan.P >= 2).
 cudaError_t launch_wilson_sech2_f32(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s);
+// FP32, flux tube (eq. (68)), phi_cm == NULL: the packed-FP32 kernel of wl_wilson_fluxtube_f32.cu (plan.P >= 2).
+cudaError_t launch_wilson_fluxtube_f32(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s);
 // FP64, sech^2, phi_cm == NULL: the lean FP64 kernel of wl_wilson_sech2_f64.cu (plan.P = 1 or 2).
 cudaError_t launch_wilson_sech2_f64(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s);
 cudaError_t launch_group_reduce(const double* partial, int64_t n_units, int units_per_group, int n_groups,
