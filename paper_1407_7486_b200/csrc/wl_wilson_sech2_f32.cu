@@ -191,7 +191,6 @@ k_wilson_sech2_f32(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit, int6
                         const u64 ip = mul2(i12n, Dmn);                           //  1/(1+E_p)
                         const u64 imn = mul2(i12n, Dp);                           // -1/(1+E_m)
                         sp[q] = fma2(mul2(Ep, ip), ip, sp[q]);                    // E_p/(1+E_p)^2 = sech^2/4
-                        const u64 fn = mul2(Em, imn);                             // -E_m/(1+E_m)
                         u64 br;                                                   // (1 - log2(1+E_m)) - u' E_m/(1+E_m)
                         if (LOGPOLY) {
                             // 1 - log2(1+E), E in [0,1]: gen_h_poly.py L 8, abs. error 6e-8
@@ -203,12 +202,13 @@ k_wilson_sech2_f32(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit, int6
                             L = fma2(L, Em, pk(-0.478176441505f, -0.478176441505f));
                             L = fma2(L, Em, pk(0.721095768202f, 0.721095768202f));
                             L = fma2(L, Em, pk(-1.44268585129f, -1.44268585129f));
-                            L = fma2(L, Em, pk(0.999999943578f, 0.999999943578f));
-                            br = fma2(um, fn, L);
+                            // last Horner step folded with the second term: 1 - log2(1+E) = c0 + E L'(E) and
+                            // -u' E/(1+E) = E (u' imn), so br = c0 + E (L' + u' imn): one instruction fewer
+                            br = fma2(fma2(um, imn, L), Em, pk(0.999999943578f, 0.999999943578f));
                         } else {
                             float dm0, dm1;
                             upk(Dmn, dm0, dm1);
-                            br = sub2(fma2(um, fn, one2), pk(xu_lg2_abs(dm0), xu_lg2_abs(dm1)));
+                            br = sub2(fma2(um, mul2(Em, imn), one2), pk(xu_lg2_abs(dm0), xu_lg2_abs(dm1)));
                         }
                         const u64 hE = mul2(br, mul2(rm, rm));                    // br / w'
                         u64 hP = fma2(h4, wm, h3);

@@ -75,13 +75,14 @@ __device__ __forceinline__ double exp2_neg(double u)
     return __hiloint2double(__double2hiint(p) - (n << 20), __double2loint(p));
 }
 
-// 1 - log2(1+E), E in [0,1]: degree-20 polynomial.
-__device__ __forceinline__ double one_minus_log2_1p(double E)
+// (1 - log2(1+E)) - u E/(1+E) for E in [0,1], im = 1/(1+E).  With the degree-20 polynomial
+// 1 - log2(1+E) = c0 + E L'(E) the second term joins the last Horner step: c0 + E (L'(E) - u im).
+__device__ __forceinline__ double bracket(double E, double u, double im)
 {
     double L = kLog[0];
 #pragma unroll
-    for (int i = 1; i < 21; ++i) L = fma(L, E, kLog[i]);
-    return L;
+    for (int i = 1; i < 20; ++i) L = fma(L, E, kLog[i]);
+    return fma(fma(-u, im, L), E, kLog[20]);
 }
 
 }  // namespace
@@ -191,7 +192,7 @@ k_wilson_sech2_f64(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit, int6
                     r = fma(r, e, r);
                     const double ip = r * Dm, im = r * Dp;
                     sp[j] = fma(Ep * ip, ip, sp[j]);                          // E_p/(1+E_p)^2 = sech^2/4
-                    const double br = fma(-um, Em * im, one_minus_log2_1p(Em));   // (1 - log2(1+E_m)) - u' E_m/(1+E_m)
+                    const double br = bracket(Em, um, im);                    // (1 - log2(1+E_m)) - u' E_m/(1+E_m)
                     const double hE = br * (irm * irm);                       // br / w'
                     // h(w)/(4 log2 e) in w', w = u^2 < 1/16 (gen_h_poly.py hs 0.0625 7)
                     double hP = kHPoly[0];
