@@ -40,7 +40,7 @@ UNIT = "point-evals/s"
 ALG_PLAIN_OPS = 29
 ALG_SFU_OPS = 7
 ALG_OPS_UNIFORM = 4
-ALG_F64_OPS_SECH2 = 98            # FP64-pipe lane-ops per point-eval, branch-free formulation
+ALG_F64_OPS_SECH2 = 97            # FP64-pipe lane-ops per point-eval, branch-free formulation
 SM_COUNT = 148
 ISSUE_LANES_PER_CLK_SM = 128      # 4 sub-partitions x 1 warp instruction (32 lanes) per clock
 FP64_LANES_PER_CLK_SM = 64        # measured 63.8 (profiles/r01_pipe_rates.md)
@@ -353,10 +353,10 @@ def run_ours(args, cfg):
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_wilson launch from the `ncu --set full` capture
 # summarised under profiles/ (per launch, like `achieved`); None until measured for that workload.
 NCU_TRAFFIC_BYTES = {
-    # profiles/r01_wilson_f32_ncu.md: 279.8 MB read (the 268.4 MB ensemble once) + 58.4 MB written (partials)
-    ("cfg3_paper_scale", "f32"): 279834624 + 58382848,
+    # profiles/r01_wilson_f32_ncu.md: 276.9 MB read (the 268.4 MB ensemble once) + 56.5 MB written (partials)
+    ("cfg3_paper_scale", "f32"): 276931072 + 56459264,
     # profiles/r01_wilson_f64_ncu.md: 4.2 MB read, partials still in L2
-    ("cfg1_small_sech2", "f64"): 4216832,
+    ("cfg1_small_sech2", "f64"): 4217088,
 }
 
 

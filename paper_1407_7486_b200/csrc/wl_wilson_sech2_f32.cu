@@ -22,8 +22,8 @@
 //   h(u)    = ln2 [ (1 - log2(1+E)) - u' E/(1+E) ] / u^2  = 4 log2(e) * br / w'
 //   m x d   = (k^2 s c) dy + (k^2 T) (y_i x y_{i+1})       = k^2 (m x d)
 // hence phase = eB0 * lambda^2 ln2 * sum_i [br/w'](i) * [k^2 m x d](i): the constants leave the loop.
-// Near the axis (w = u^2 < 1/4) the bracket cancels and a degree-4 polynomial in w' replaces br/w'
-// (coefficients: gen_h_poly.py hs 0.25 4, relative error 5e-8).
+// Near the axis (w = u^2 < 1/8) the bracket cancels and a degree-3 polynomial in w' replaces br/w'
+// (coefficients: gen_h_poly.py hs 0.125 3, relative error 8e-8).
 #include "wl_internal.cuh"
 
 namespace wl {
@@ -95,11 +95,10 @@ k_wilson_sech2_f32(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit, int6
     }
     const u64 one2 = pk(1.0f, 1.0f), mone2 = pk(-1.0f, -1.0f);
     constexpr float kTiny = 1e-36f;                 // rsqrt(kTiny)^2 is still finite
-    constexpr float kPolyBelow = 2.0813689810f;     // w' < this  <=>  u^2 < 1/4
-    // h(w)/(4 log2 e) in w' (gen_h_poly.py hs 0.25 4)
-    const u64 h0 = pk(0.0866433954731f, 0.0866433954731f), h1 = pk(-0.005203459712f, -0.005203459712f),
-              h2 = pk(0.000277586359849f, 0.000277586359849f), h3 = pk(-1.39101401155e-5f, -1.39101401155e-5f),
-              h4 = pk(5.53576426559e-7f, 5.53576426559e-7f);
+    constexpr float kPolyBelow = 1.0406844905f;     // w' < this  <=>  u^2 < 1/8
+    // h(w)/(4 log2 e) in w' (gen_h_poly.py hs 0.125 3, rel. error 8e-8)
+    const u64 h0 = pk(0.086643391691228f, 0.086643391691228f), h1 = pk(-0.0052033291295960f, -0.0052033291295960f),
+              h2 = pk(0.00027690498335525f, 0.00027690498335525f), h3 = pk(-1.2801479229129e-5f, -1.2801479229129e-5f);
 
     constexpr int kLevels = DISC ? 3 : 1;
     double Wsum[kLevels][P];
@@ -211,8 +210,7 @@ k_wilson_sech2_f32(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit, int6
                             br = sub2(fma2(um, mul2(Em, imn), one2), pk(xu_lg2_abs(dm0), xu_lg2_abs(dm1)));
                         }
                         const u64 hE = mul2(br, mul2(rm, rm));                    // br / w'
-                        u64 hP = fma2(h4, wm, h3);
-                        hP = fma2(hP, wm, h2);
+                        u64 hP = fma2(h3, wm, h2);
                         hP = fma2(hP, wm, h1);
                         hP = fma2(hP, wm, h0);
                         float hE0, hE1, hP0, hP1;
