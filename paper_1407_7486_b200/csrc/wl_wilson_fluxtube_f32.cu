@@ -200,23 +200,25 @@ k_wilson_fluxtube_f32(EvalArgs a, int n_grid, int n_tiles, int loops_per_unit, i
 cudaError_t launch_wilson_fluxtube_f32(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s)
 {
     const size_t smem = (sizeof(float4) + sizeof(float2)) * (size_t)kChunk;
-    const int64_t n_ctas = plan.n_units * plan.n_tiles;
+    // Grids of at most 256 points: 128 threads x 2 grid points, so that no thread of the tile idles.
+    const bool small = plan.n_grid <= 256;
+    const int n_tiles = small ? 1 : plan.n_tiles;
+    const int64_t n_ctas = plan.n_units * n_tiles;
     if (n_ctas > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     const unsigned g = (unsigned)n_ctas;
-    // 256 threads x P = 4, 4 CTAs/SM, inner loop unrolled by 2, as k_wilson_sech2_f32.
-#define WL_LAUNCH(PP, DD) k_wilson_fluxtube_f32<PP, kThreads, 4, 2, kSumBlock, DD><<<g, kThreads, smem, s>>>(a, plan.n_grid, plan.n_tiles, plan.loops_per_unit, plan.n_units)
+    // 256 threads x P = 4, 4 CTAs/SM (64 registers), inner loop unrolled by 2: the fastest of the
+    // combinations measured (profiles/r01_variants.md).
+#define WL_LAUNCH(PP, TH, DD) k_wilson_fluxtube_f32<PP, TH, 4, 2, kSumBlock, DD><<<g, TH, smem, s>>>(a, plan.n_grid, n_tiles, plan.loops_per_unit, plan.n_units)
     if (a.disc) {
-        switch (plan.P) {
-            case 2: WL_LAUNCH(2, true); break;
-            case 4: WL_LAUNCH(4, true); break;
-            default: return cudaErrorInvalidValue;
-        }
+        if (small) WL_LAUNCH(2, 128, true);
+        else if (plan.P == 2) WL_LAUNCH(2, kThreads, true);
+        else if (plan.P == 4) WL_LAUNCH(4, kThreads, true);
+        else return cudaErrorInvalidValue;
     } else {
-        switch (plan.P) {
-            case 2: WL_LAUNCH(2, false); break;
-            case 4: WL_LAUNCH(4, false); break;
-            default: return cudaErrorInvalidValue;
-        }
+        if (small) WL_LAUNCH(2, 128, false);
+        else if (plan.P == 2) WL_LAUNCH(2, kThreads, false);
+        else if (plan.P == 4) WL_LAUNCH(4, kThreads, false);
+        else return cudaErrorInvalidValue;
     }
 #undef WL_LAUNCH
     return cudaGetLastError();
