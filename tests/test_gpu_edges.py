@@ -218,3 +218,37 @@ def test_error_statuses(api):
     mean, _ = api.wl_eval(f, loops, T, rho, None, n_groups=2, compute="f64")
     torch.cuda.synchronize()
     assert torch.all(torch.isfinite(mean))
+
+
+def test_eval_and_finalize_capture_into_a_cuda_graph(api):
+    """include/wl.h: no call except wl_eval_host allocates, copies or synchronises -- so the whole step
+    (wl_eval + wl_jackknife_finalize, 4 kernels) can be captured once and replayed as a CUDA graph."""
+    c = inputs.config(1)
+    T, rho, _ = c.grids()
+    loops = api.wl_loops_generate(c.n_loops, c.n_ppl, c.seed, torch.float32)
+    f = api.wl_field_create(c.profile, c.params)
+    Td, rd = dev(T), dev(rho)
+    n_grid = len(T) * len(rho)
+    W_mean = torch.empty((len(T), len(rho)), dtype=torch.float64, device="cuda")
+    gs = torch.empty((c.n_groups, len(T), len(rho)), dtype=torch.float64, device="cuda")
+    ws = torch.empty(api.wl_eval_workspace_bytes(c.n_loops, c.n_ppl, len(T), len(rho), c.n_groups, "f32"),
+                     dtype=torch.uint8, device="cuda")
+    ref_mean, ref_gs = api.wl_eval(f, loops, Td, rd, None, n_groups=c.n_groups, compute="f32")
+    ref_fm, ref_err = api.wl_jackknife_finalize(ref_gs, c.n_loops)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(graph, stream=side):
+            api.wl_eval(f, loops, Td, rd, None, n_groups=c.n_groups, compute="f32", W_mean=W_mean, group_sums=gs,
+                        workspace=ws, stream=side)
+            fm, err = api.wl_jackknife_finalize(gs, c.n_loops, stream=side)
+    W_mean.zero_()
+    gs.zero_()
+    for _ in range(3):
+        graph.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(W_mean, ref_mean) and torch.equal(gs, ref_gs)
+    assert torch.equal(fm, ref_fm) and torch.equal(err, ref_err)
+    assert n_grid == 256
