@@ -28,6 +28,10 @@
  * (eq. (68)) and the scalar-QED output W = cos(phase), pinned
  * in tests/test_oracle_fluxtube_scalar.py.
  *
+ * Also (NEXT-4): the Q-point Gauss-Legendre rule for the t-integral of eq. (24) (wlo_loop_phase_spin_q,
+ * pinned in tests/test_oracle_quadrature.py) and shuffled group assignment per proper time (wlo_shuffle_index,
+ * wlo_regroup_shuffled; pinned in tests/test_oracle_shuffle.py).
+ *
  * Pins (tests/test_oracle_*.py, all -m "not gpu"): zero field, uniform-field
  * shoelace area, finite-N uniform closed form, Stokes flux of the sech^2
  * profile by independent quadrature, mpmath evaluation of the profile,
@@ -188,6 +192,114 @@ int wlo_eval_particle(int profile, const double *params, int scalar,
             }
     }
 
+    for (int64_t k = 0; k < n_grid; ++k) {
+        double total = 0.0;
+        for (int g = 0; g < n_groups; ++g) {
+            double S = 0.0;
+            for (int64_t l = g * per_group; l < (g + 1) * per_group; ++l) S += W[l * n_grid + k];
+            group_sums[(int64_t)g * n_grid + k] = S;
+            total += S;
+        }
+        W_mean[k] = total / (double)n_loops;
+    }
+    if (!W_loop) free(W);
+    return 0;
+}
+
+/* ------------------------------------------------------------------------- */
+/* Higher-order quadrature of the t-integral of eq. (24) (SURVEY.md 8(f)      */
+/* NEXT-4; "in general, we wish to compute these integrals  */
+/* numerically ... gauge invariance ... can be preserved to any numerical     */
+/* precision that's desired").  Segment i contributes, eq. (24),              */
+/*   (x^i y^{i+1} - y^i x^{i+1}) int_0^1 dt g(rho_i(t)),                      */
+/*   rho_i^2(t) = A_i + 2 B_i t + C_i t^2,                    eq. (25)         */
+/*   A_i = |x^i|^2, B_i = x^i . (x^{i+1} - x^i), C_i = |x^{i+1} - x^i|^2       */
+/*                                                            eq. (26)-(28)    */
+/* with g(rho) = F f_lambda(rho^2)/rho^2 = e A_phi/rho (eq. (23)), and the     */
+/* t-integral is taken by the Q-point Gauss-Legendre rule on [0, 1]:           */
+/*   Q = 1: t = 1/2 (the midpoint rule of wlo_loop_phase_spin),                */
+/*   Q = 2: t = 1/2 -+ 1/(2 sqrt 3),            weights 1/2, 1/2,              */
+/*   Q = 3: t = 1/2 -+ sqrt(3/5)/2, 1/2,        weights 5/18, 4/9, 5/18.       */
+/* The spin factor is the point-sampled sum of wlo_loop_phase_spin (north_star).*/
+/* Returns 0, or -1 if Q is not 1, 2 or 3.                                     */
+/* ------------------------------------------------------------------------- */
+int wlo_gauss_legendre_01(int Q, double *t, double *w)
+{
+    if (Q == 1) { t[0] = 0.5; w[0] = 1.0; return 0; }
+    if (Q == 2) {
+        double d = 0.5 / sqrt(3.0);
+        t[0] = 0.5 - d; t[1] = 0.5 + d; w[0] = 0.5; w[1] = 0.5;
+        return 0;
+    }
+    if (Q == 3) {
+        double d = 0.5 * sqrt(3.0 / 5.0);
+        t[0] = 0.5 - d; t[1] = 0.5; t[2] = 0.5 + d;
+        w[0] = 5.0 / 18.0; w[1] = 4.0 / 9.0; w[2] = 5.0 / 18.0;
+        return 0;
+    }
+    return -1;
+}
+
+int wlo_loop_phase_spin_q(int profile, const double *params,
+                          const double *y, int N, double T, double cx, double cy, int Q,
+                          double *phase_out, double *spin_out)
+{
+    double tq[3], wq[3];
+    if (wlo_gauss_legendre_01(Q, tq, wq) != 0) return -1;
+    double s = sqrt(T);
+    double phase = 0.0, spin = 0.0;
+    for (int i = 0; i < N; ++i) {
+        int j = (i + 1) % N;
+        double xi = cx + s * y[2 * i], yi = cy + s * y[2 * i + 1];
+        double xj = cx + s * y[2 * j], yj = cy + s * y[2 * j + 1];
+        double A = xi * xi + yi * yi;                                   /* eq. (26) */
+        double B = xi * (xj - xi) + yi * (yj - yi);                     /* eq. (27) */
+        double Cc = (xj - xi) * (xj - xi) + (yj - yi) * (yj - yi);      /* eq. (28) */
+        double integral = 0.0;
+        for (int q = 0; q < Q; ++q) {
+            double rho2 = A + 2.0 * B * tq[q] + Cc * tq[q] * tq[q];     /* eq. (25) */
+            if (rho2 < 0.0) rho2 = 0.0;                                 /* rounding, segment through the axis */
+            integral += wq[q] * wlo_field_g(profile, params, sqrt(rho2));
+        }
+        phase += (xi * yj - yi * xj) * integral;                        /* eq. (24) */
+        spin += wlo_field_b(profile, params, sqrt(xi * xi + yi * yi));
+    }
+    *phase_out = phase;
+    *spin_out = T / (double)N * spin;
+    return 0;
+}
+
+/* wlo_eval_particle with the Q-point rule for eq. (24); same outputs, same group order. */
+int wlo_eval_quadrature(int profile, const double *params, int scalar, int Q,
+             const double *loops, int64_t n_loops, int N,
+             const double *T, int n_T,
+             const double *rho_cm, const double *phi_cm, int n_rho,
+             int n_groups,
+             double *W_mean, double *group_sums,
+             double *W_loop, double *phase_loop, double *spin_loop)
+{
+    if (n_loops <= 0 || N < 1 || n_T < 1 || n_rho < 1 || n_groups < 1) return -1;
+    if (n_loops % n_groups != 0 || Q < 1 || Q > 3) return -1;
+    const int64_t n_grid = (int64_t)n_T * n_rho;
+    const int64_t per_group = n_loops / n_groups;
+    double *W = W_loop ? W_loop : (double *)malloc(sizeof(double) * n_loops * n_grid);
+    if (!W) return -1;
+
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t l = 0; l < n_loops; ++l) {
+        const double *y = loops + l * (int64_t)N * 2;
+        for (int t = 0; t < n_T; ++t)
+            for (int r = 0; r < n_rho; ++r) {
+                double ph = phi_cm ? phi_cm[r] : 0.0;
+                double cx = rho_cm[r] * cos(ph), cy = rho_cm[r] * sin(ph);
+                double phase, spin;
+                wlo_loop_phase_spin_q(profile, params, y, N, T[t], cx, cy, Q, &phase, &spin);
+                int64_t o = l * n_grid + (int64_t)t * n_rho + r;
+                W[o] = scalar ? cos(phase) : cos(phase) * cosh(spin);
+                if (phase_loop) phase_loop[o] = phase;
+                if (spin_loop) spin_loop[o] = spin;
+            }
+    }
     for (int64_t k = 0; k < n_grid; ++k) {
         double total = 0.0;
         for (int g = 0; g < n_groups; ++g) {
@@ -441,6 +553,78 @@ void wlo_normal_pair(uint64_t seed, uint64_t loop, uint32_t point, double *nx, d
     double th = 6.283185307179586476925286766559 * u2;
     *nx = r * cos(th);
     *ny = r * sin(th);
+}
+
+/* ------------------------------------------------------------------------- */
+/* Shuffled group assignment (Sec. IV.B.3,             */
+/* PAPER.md:411-417, Fig. 6 at PAPER.md:380): "randomize how worldlines are    */
+/* assigned to groups between each evaluation of the integrand".  One          */
+/* evaluation of the integrand = one proper time T_t, so every T index t gets  */
+/* its own seeded permutation pi_t of the loops, and group g at that T is      */
+/*   { pi_t(i) : g N_l/G <= i < (g+1) N_l/G },  summed in the order of i       */
+/* (reading A17).  pi_t is a keyed bijection of [0, n_loops): a      */
+/* balanced Feistel network of 6 rounds on 2b bits (b the smallest integer     */
+/* with 4^b >= n_loops) whose round function is word 0 of Philox4x32-10 with   */
+/* counter (R, round, t, 0x5348464C) and key (seed_lo, seed_hi), followed by   */
+/* cycle walking (apply again while the image is >= n_loops).  A Feistel       */
+/* network is a bijection of [0, 4^b) whatever its round function, and cycle   */
+/* walking restricts a bijection to a bijection of the subset.                 */
+/* ------------------------------------------------------------------------- */
+int64_t wlo_shuffle_index(uint64_t seed, int t, int64_t n_loops, int64_t i)
+{
+    int b = 1;
+    while (((int64_t)1 << (2 * b)) < n_loops) ++b;
+    const uint32_t mask = (uint32_t)(((uint64_t)1 << b) - 1u);
+    const uint32_t key[2] = { (uint32_t)seed, (uint32_t)(seed >> 32) };
+    uint64_t x = (uint64_t)i;
+    do {
+        uint32_t L = (uint32_t)(x >> b), R = (uint32_t)(x & mask);
+        for (uint32_t round = 0; round < 6; ++round) {
+            uint32_t ctr[4] = { R, round, (uint32_t)t, 0x5348464Cu };
+            uint32_t w[4];
+            wlo_philox4x32_10(ctr, key, w);
+            uint32_t nR = L ^ (w[0] & mask);
+            L = R;
+            R = nR;
+        }
+        x = ((uint64_t)L << b) | R;
+    } while (x >= (uint64_t)n_loops);
+    return (int64_t)x;
+}
+
+/* perm[t][i] = pi_t(i), [n_T][n_loops]. */
+int wlo_group_permutation(uint64_t seed, int64_t n_loops, int n_T, int64_t *perm)
+{
+    if (n_loops < 1 || n_T < 1) return -1;
+    for (int t = 0; t < n_T; ++t)
+        for (int64_t i = 0; i < n_loops; ++i)
+            perm[(int64_t)t * n_loops + i] = wlo_shuffle_index(seed, t, n_loops, i);
+    return 0;
+}
+
+/* Group sums and mean from per-loop W [n_loops][n_T][n_rho] with the groups of table perm[n_T][n_loops]:
+ * S_g[t][r] = sum_{i = g N_l/G}^{(g+1) N_l/G - 1} W[perm[t][i]][t][r]  (eq. (60) with shuffled membership),
+ * <W>[t][r] = (sum_g S_g[t][r])/N_l  (eq. (61)-(62): unchanged by the grouping, up to rounding). */
+int wlo_regroup_shuffled(const double *W_loop, int64_t n_loops, int n_T, int n_rho, int n_groups,
+                         const int64_t *perm, double *group_sums, double *W_mean)
+{
+    if (n_loops < 1 || n_T < 1 || n_rho < 1 || n_groups < 1 || n_loops % n_groups != 0) return -1;
+    const int64_t n_grid = (int64_t)n_T * n_rho;
+    const int64_t per_group = n_loops / n_groups;
+    for (int t = 0; t < n_T; ++t)
+        for (int r = 0; r < n_rho; ++r) {
+            int64_t k = (int64_t)t * n_rho + r;
+            double total = 0.0;
+            for (int g = 0; g < n_groups; ++g) {
+                double S = 0.0;
+                for (int64_t i = g * per_group; i < (g + 1) * per_group; ++i)
+                    S += W_loop[perm[(int64_t)t * n_loops + i] * n_grid + k];
+                group_sums[(int64_t)g * n_grid + k] = S;
+                total += S;
+            }
+            W_mean[k] = total / (double)n_loops;
+        }
+    return 0;
 }
 
 /* d-loop generator.  Step (1): y_N = 0 (stored at index 0).

@@ -61,6 +61,20 @@ def lib():
         L.wlo_generate_loops.restype = C.c_int
         L.wlo_generate_loops.argtypes = [C.c_uint64, C.c_int64, C.c_int64, C.c_int, _dp]
         L.wlo_num_threads.restype = C.c_int
+        L.wlo_gauss_legendre_01.restype = C.c_int
+        L.wlo_gauss_legendre_01.argtypes = [C.c_int, _dp, _dp]
+        L.wlo_loop_phase_spin_q.restype = C.c_int
+        L.wlo_loop_phase_spin_q.argtypes = [C.c_int, _dp, _dp, C.c_int, C.c_double, C.c_double, C.c_double, C.c_int,
+                                            _dp, _dp]
+        L.wlo_eval_quadrature.restype = C.c_int
+        L.wlo_eval_quadrature.argtypes = [C.c_int, _dp, C.c_int, C.c_int, _dp, C.c_int64, C.c_int, _dp, C.c_int, _dp,
+                                          _dp, C.c_int, C.c_int, _dp, _dp, _dp, _dp, _dp]
+        L.wlo_shuffle_index.restype = C.c_int64
+        L.wlo_shuffle_index.argtypes = [C.c_uint64, C.c_int, C.c_int64, C.c_int64]
+        L.wlo_group_permutation.restype = C.c_int
+        L.wlo_group_permutation.argtypes = [C.c_uint64, C.c_int64, C.c_int, C.POINTER(C.c_int64)]
+        L.wlo_regroup_shuffled.restype = C.c_int
+        L.wlo_regroup_shuffled.argtypes = [_dp, C.c_int64, C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int64), _dp, _dp]
         _lib = L
     return _lib
 
@@ -128,6 +142,81 @@ def evaluate(profile, params, loops, T, rho_cm, phi_cm=None, n_groups=1, per_loo
     if per_loop:
         out.update(W=W, phase=ph, spin=sp)
     return out
+
+
+def gauss_legendre_01(Q):
+    """(nodes, weights) of the Q-point Gauss-Legendre rule on [0, 1] as the oracle uses them (Q = 1, 2, 3)."""
+    t, w = np.empty(3), np.empty(3)
+    if lib().wlo_gauss_legendre_01(int(Q), _p(t), _p(w)) != 0:
+        raise ValueError("Q must be 1, 2 or 3")
+    return t[:Q].copy(), w[:Q].copy()
+
+
+def loop_phase_spin_q(profile, params, y, T, cx, cy, Q):
+    """(phase, spin) of one unit loop with the Q-point rule for the t-integral of eq. (24), eq. (25)-(28)."""
+    pr = _f64(params)
+    y = _f64(y)
+    assert y.ndim == 2 and y.shape[1] == 2
+    ph, sp = C.c_double(), C.c_double()
+    if lib().wlo_loop_phase_spin_q(profile, _p(pr), _p(y), y.shape[0], float(T), float(cx), float(cy), int(Q),
+                                   C.byref(ph), C.byref(sp)) != 0:
+        raise ValueError("Q must be 1, 2 or 3")
+    return ph.value, sp.value
+
+
+def evaluate_quadrature(profile, params, loops, T, rho_cm, phi_cm=None, n_groups=1, per_loop=False, scalar=False,
+                        Q=1):
+    """`evaluate` with the Q-point Gauss-Legendre rule for the t-integral of eq. (24)."""
+    pr = _f64(params)
+    y = _f64(loops)
+    assert y.ndim == 3 and y.shape[2] == 2
+    T = _f64(T)
+    rho = _f64(rho_cm)
+    phi = _f64(phi_cm) if phi_cm is not None else None
+    nl, N = y.shape[0], y.shape[1]
+    nT, nr = T.shape[0], rho.shape[0]
+    mean = np.empty((nT, nr))
+    gs = np.empty((n_groups, nT, nr))
+    W = ph = sp = None
+    if per_loop:
+        W, ph, sp = (np.empty((nl, nT, nr)) for _ in range(3))
+    rc = lib().wlo_eval_quadrature(profile, _p(pr), 1 if scalar else 0, int(Q), _p(y), nl, N, _p(T), nT, _p(rho),
+                                   _p(phi), nr, n_groups, _p(mean), _p(gs), _p(W), _p(ph), _p(sp))
+    if rc != 0:
+        raise ValueError("wlo_eval_quadrature: invalid argument")
+    out = {"W_mean": mean, "group_sums": gs}
+    if per_loop:
+        out.update(W=W, phase=ph, spin=sp)
+    return out
+
+
+def shuffle_index(seed, t, n_loops, i):
+    """pi_t(i): the loop at position i of the shuffled order used at proper-time index t."""
+    return int(lib().wlo_shuffle_index(int(seed), int(t), int(n_loops), int(i)))
+
+
+def group_permutation(seed, n_loops, n_T):
+    """perm [n_T][n_loops] (int64): perm[t][i] = pi_t(i)."""
+    perm = np.empty((n_T, n_loops), dtype=np.int64)
+    if lib().wlo_group_permutation(int(seed), int(n_loops), int(n_T),
+                                   perm.ctypes.data_as(C.POINTER(C.c_int64))) != 0:
+        raise ValueError("wlo_group_permutation: invalid argument")
+    return perm
+
+
+def regroup_shuffled(W_loop, n_groups, perm):
+    """(W_mean [n_T][n_rho], group_sums [G][n_T][n_rho]) from per-loop W [n_loops][n_T][n_rho] with the
+    per-T group membership of `perm` [n_T][n_loops] (eq. (60) with shuffled groups)."""
+    W = _f64(W_loop)
+    nl, nT, nr = W.shape
+    perm = np.ascontiguousarray(perm, dtype=np.int64)
+    assert perm.shape == (nT, nl)
+    mean = np.empty((nT, nr))
+    gs = np.empty((n_groups, nT, nr))
+    if lib().wlo_regroup_shuffled(_p(W), nl, nT, nr, int(n_groups), perm.ctypes.data_as(C.POINTER(C.c_int64)),
+                                  _p(gs), _p(mean)) != 0:
+        raise ValueError("wlo_regroup_shuffled: invalid argument")
+    return mean, gs
 
 
 def evaluate_discretization(profile, params, loops, T, rho_cm, phi_cm=None, n_groups=1, per_loop=False,
