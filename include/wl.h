@@ -27,7 +27,8 @@
  *   - All grids and results are FP64.  Loop coordinates are FP32 or FP64,
  *     array-of-points: loops[l][i][c], c = 0 (x), 1 (y), contiguous.
  *   - Every call returns a wl_status; nothing is printed, nothing aborts.
- *     On any status other than WL_OK no kernel has been launched by that call.
+ *     Argument errors (WL_ERR_INVALID_ARG, WL_ERR_UNSUPPORTED, WL_ERR_WORKSPACE) are found before
+ *     anything is enqueued; on any status other than WL_OK no result buffer is valid.
  *     (The paper's convention is "check the code, print the string",
  *     PAPER.md:603-628; wl_status_string gives the string.)
  *   - There is no CPU fallback: without a CUDA device the compute calls
@@ -92,7 +93,7 @@ void wl_field_destroy(wl_field* field);   /* NULL is allowed */
  * d_loops[n_loops][n_ppl][2] in `storage` precision (arithmetic is FP64; FP32
  * storage rounds once at the store).  Loop l of an ensemble is the same whatever
  * loop_begin / n_loops window it is generated in.
- * n_ppl: power of two, 2 <= n_ppl <= 8192.  n_loops == 0 is a no-op.  */
+ * n_ppl: power of two, 2 <= n_ppl <= 65536.  n_loops == 0 is a no-op.  */
 wl_status wl_loops_generate(void* d_loops, wl_dtype storage, int64_t loop_begin, int64_t n_loops,
                             int n_ppl, uint64_t seed, void* stream);
 
@@ -107,13 +108,14 @@ size_t wl_eval_workspace_bytes(int64_t n_loops, int n_ppl, int n_T, int n_rho, i
  *   d_group_sums[g][t][r] = S_g, group g = loops [g n_loops/G, (g+1) n_loops/G)
  * d_loops [n_loops][n_ppl][2] of loop_dtype; n_ppl >= 1 (any value, not only
  * powers of two).  d_T[n_T] > 0; d_rho_cm[n_rho] >= 0; d_phi_cm[n_rho] or NULL
- * (= all zero).  Grid VALUES are not read on the host and are not validated.
+ * (= all zero).  Grid VALUES live on the device and are not read by this call: T <= 0 or a
+ * non-finite value gives NaN rows, not an error.  wl_grid_validate checks a host copy.
  * compute = WL_F64: all arithmetic FP64.  compute = WL_F32: per-term arithmetic
  * FP32 with fast intrinsics, the sums round a loop accumulated in FP64 from
  * FP32 partials of 32 terms, cos/cosh and all sums over loops FP64.
  * Errors: null pointers, sizes < 1, n_groups < 1, n_loops % n_groups != 0
- * (equal groups are required) -> WL_ERR_INVALID_ARG; workspace
- * too small -> WL_ERR_WORKSPACE. */
+ * (equal groups are required), n_T * n_rho > 2^24, more than 2^31 - 1 CTAs
+ * -> WL_ERR_INVALID_ARG; workspace too small -> WL_ERR_WORKSPACE. */
 wl_status wl_eval(const wl_field* field,
                   const void* d_loops, wl_dtype loop_dtype, int64_t n_loops, int n_ppl,
                   const double* d_T, int n_T,
@@ -121,6 +123,96 @@ wl_status wl_eval(const wl_field* field,
                   int n_groups, wl_dtype compute,
                   double* d_W_mean, double* d_group_sums,
                   void* d_workspace, size_t workspace_bytes, void* stream);
+
+/* Host helper: WL_OK if every h_T[k] is finite and > 0 and every h_rho_cm[k] is finite and >= 0
+ * ("T <= 0, negative rho_cm -> invalid"), else WL_ERR_INVALID_ARG.
+ * The evaluation calls take DEVICE grids and cannot check them without a synchronisation. */
+wl_status wl_grid_validate(const double* h_T, int n_T, const double* h_rho_cm, int n_rho);
+
+/* ---- Options of the extended evaluation calls ------------------
+ *
+ * quadrature_order (eq. (24)-(28)): number Q of Gauss-Legendre points in t for
+ *   int_0^1 dt f(rho_i^2(t))/rho_i^2(t) with rho_i^2(t) = A_i + 2 B_i t + C_i t^2 (eq. (25)):
+ *   0 or 1 = the one-point midpoint rule of wl_eval; 2: t = 1/2 -+ 1/(2 sqrt 3), weights 1/2;
+ *   3: t = 1/2 -+ sqrt(3/5)/2, 1/2, weights 5/18, 4/9, 5/18.  The spin sum is unchanged.
+ *   Q > 1 together with the discretisation estimate -> WL_ERR_UNSUPPORTED.
+ *
+ * seeded ("generating the loops on-the-fly directly on the GPU device itself without
+ *   storing the entire loop in memory", the device-memory ceiling): non-zero = d_loops
+ *   is ignored (may be NULL); loop l is regenerated inside the kernel as loop (loop_begin + l) of
+ *   the ensemble `seed`, exactly as wl_loops_generate would have stored it in `loop_dtype`
+ *   precision: the results have the same bits as wl_loops_generate followed by wl_eval.
+ *   n_ppl must be a power of two, 2 <= n_ppl <= 65536.
+ *
+ * shuffle_groups (Sec. IV.B.3; Fig. 6: "randomize how worldlines are
+ *   assigned to groups between each evaluation of the integrand"): non-zero = every proper-time
+ *   index t has its own permutation pi_t of the loops (see wl_group_permutation) and group g at
+ *   that T holds the loops pi_t(i), g n_loops/G <= i < (g+1) n_loops/G, summed in the order of i.
+ *   <W> is unchanged up to rounding (eq. (61)-(62)).  Needs n_loops < 2^31 and the larger
+ *   workspace of wl_eval_opt_workspace_bytes (all per-loop W values are kept: 8 n_loops n_T n_rho bytes).
+ *
+ * staging: 0 = loop chunks are read by ordinary coalesced loads; 1 = by cp.async.bulk into a
+ *   two-slot shared-memory ring with mbarrier completion, one chunk ahead of the evaluation
+ *   (compiled for the main kernels only, silently 0 elsewhere; same bits either way).
+ *
+ * event_wilson_begin / event_wilson_end: optional cudaEvent_t (as void*) recorded on the stream
+ *   immediately before and after the k_wilson launch. */
+typedef struct wl_eval_options {
+    size_t struct_size;          /* sizeof(wl_eval_options): set by wl_eval_options_default */
+    int quadrature_order;
+    int seeded;
+    uint64_t seed;
+    int64_t loop_begin;
+    int shuffle_groups;
+    int staging;
+    uint64_t shuffle_seed;
+    void* event_wilson_begin;
+    void* event_wilson_end;
+} wl_eval_options;
+
+/* Fills *opt with the defaults (= plain wl_eval).  NULL is ignored. */
+void wl_eval_options_default(wl_eval_options* opt);
+
+/* wl_eval with options (opt == NULL: exactly wl_eval).  Workspace: wl_eval_opt_workspace_bytes
+ * (0 on invalid sizes or options).  Errors as wl_eval; an unknown quadrature order, a struct_size
+ * that is not sizeof(wl_eval_options), seeded with a bad n_ppl -> WL_ERR_INVALID_ARG. */
+size_t wl_eval_opt_workspace_bytes(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups,
+                                   wl_dtype compute, const wl_eval_options* opt);
+wl_status wl_eval_opt(const wl_field* field,
+                      const void* d_loops, wl_dtype loop_dtype, int64_t n_loops, int n_ppl,
+                      const double* d_T, int n_T,
+                      const double* d_rho_cm, const double* d_phi_cm, int n_rho,
+                      int n_groups, wl_dtype compute,
+                      double* d_W_mean, double* d_group_sums,
+                      void* d_workspace, size_t workspace_bytes, void* stream,
+                      const wl_eval_options* opt);
+
+/* wl_eval without an ensemble buffer: loops [loop_begin, loop_begin + n_loops) of the ensemble `seed`
+ * are regenerated inside the kernel (= wl_eval_opt with seeded set).  `storage` is the
+ * precision wl_loops_generate would have stored them in.  Workspace: wl_eval_workspace_bytes. */
+wl_status wl_eval_seeded(const wl_field* field, uint64_t seed, int64_t loop_begin, wl_dtype storage,
+                         int64_t n_loops, int n_ppl,
+                         const double* d_T, int n_T,
+                         const double* d_rho_cm, const double* d_phi_cm, int n_rho,
+                         int n_groups, wl_dtype compute,
+                         double* d_W_mean, double* d_group_sums,
+                         void* d_workspace, size_t workspace_bytes, void* stream);
+
+/* wl_eval_per_loop with options (quadrature_order, seeded; shuffle_groups is ignored). */
+wl_status wl_eval_per_loop_opt(const wl_field* field,
+                               const void* d_loops, wl_dtype loop_dtype, int64_t n_loops, int n_ppl,
+                               const double* d_T, int n_T,
+                               const double* d_rho_cm, const double* d_phi_cm, int n_rho,
+                               wl_dtype compute,
+                               double* d_W, double* d_phase, double* d_spin, void* stream,
+                               const wl_eval_options* opt);
+
+/* The group-membership table of shuffle_groups: d_perm[t][i] = pi_t(i) (int32, [n_T][n_loops]).
+ * pi_t is a keyed bijection of [0, n_loops): a balanced Feistel network of 6 rounds on 2b bits (b the
+ * smallest integer with 4^b >= n_loops) whose round function is word 0 of Philox4x32-10 with counter
+ * (R, round, t, 0x5348464C) and key (seed_lo, seed_hi), applied again while the image is >= n_loops
+ * (cycle walking).  1 <= n_loops < 2^31, n_T >= 1. */
+wl_status wl_group_permutation(uint64_t shuffle_seed, int64_t n_loops, int n_T, int32_t* d_perm, void* stream);
 
 /* wl_eval with two optional CUDA events (cudaEvent_t passed as void*, NULL = none)
  * recorded on `stream` immediately before and after the k_wilson launch, so that a

@@ -46,6 +46,29 @@ _lib.wl_eval.argtypes = [_vp, _vp, _int, _i64, _int, _dp, _int, _dp, _dp, _int, 
                          _vp, _sz, _vp]
 _lib.wl_eval_instrumented.restype = _int
 _lib.wl_eval_instrumented.argtypes = list(_lib.wl_eval.argtypes) + [_vp, _vp]
+
+
+class _Options(C.Structure):
+    """struct wl_eval_options of include/wl.h."""
+    _fields_ = [("struct_size", C.c_size_t), ("quadrature_order", C.c_int), ("seeded", C.c_int),
+                ("seed", C.c_uint64), ("loop_begin", C.c_int64), ("shuffle_groups", C.c_int), ("staging", C.c_int),
+                ("shuffle_seed", C.c_uint64), ("event_wilson_begin", C.c_void_p), ("event_wilson_end", C.c_void_p)]
+
+
+_op = C.POINTER(_Options)
+_lib.wl_eval_options_default.restype = None
+_lib.wl_eval_options_default.argtypes = [_op]
+_lib.wl_eval_opt_workspace_bytes.restype = _sz
+_lib.wl_eval_opt_workspace_bytes.argtypes = [_i64, _int, _int, _int, _int, _int, _op]
+_lib.wl_eval_opt.restype = _int
+_lib.wl_eval_opt.argtypes = list(_lib.wl_eval.argtypes) + [_op]
+_lib.wl_eval_seeded.restype = _int
+_lib.wl_eval_seeded.argtypes = [_vp, _u64, _i64, _int, _i64, _int, _dp, _int, _dp, _dp, _int, _int, _int, _dp, _dp,
+                                _vp, _sz, _vp]
+_lib.wl_group_permutation.restype = _int
+_lib.wl_group_permutation.argtypes = [_u64, _i64, _int, _vp, _vp]
+_lib.wl_grid_validate.restype = _int
+_lib.wl_grid_validate.argtypes = [C.POINTER(C.c_double), _int, C.POINTER(C.c_double), _int]
 _lib.wl_eval_discretization_workspace_bytes.restype = _sz
 _lib.wl_eval_discretization_workspace_bytes.argtypes = [_i64, _int, _int, _int, _int, _int]
 _lib.wl_eval_discretization.restype = _int
@@ -63,6 +86,8 @@ _lib.wl_action_radial.argtypes = [_dp, _int, _dp, _int, _dp, _vp]
 _lib.wl_eval_per_loop.restype = _int
 _lib.wl_eval_per_loop.argtypes = [_vp, _vp, _int, _i64, _int, _dp, _int, _dp, _dp, _int, _int, _dp, _dp,
                                   _dp, _vp]
+_lib.wl_eval_per_loop_opt.restype = _int
+_lib.wl_eval_per_loop_opt.argtypes = list(_lib.wl_eval_per_loop.argtypes) + [_op]
 _lib.wl_jackknife_finalize.restype = _int
 _lib.wl_jackknife_finalize.argtypes = [_dp, _int, _i64, _int, _int, _dp, _dp, _dp, _vp]
 _lib.wl_eval_host.restype = _int
@@ -190,12 +215,38 @@ def _event_handle(ev, stream):
     return C.c_void_p(ev.cuda_event)
 
 
+def wl_eval_options(quadrature_order=1, seed=None, loop_begin=0, shuffle_seed=None, staging=0) -> _Options:
+    """struct wl_eval_options: seed != None sets `seeded`, shuffle_seed != None sets `shuffle_groups`."""
+    o = _Options()
+    _lib.wl_eval_options_default(C.byref(o))
+    o.quadrature_order = int(quadrature_order)
+    if seed is not None:
+        o.seeded, o.seed, o.loop_begin = 1, int(seed), int(loop_begin)
+    if shuffle_seed is not None:
+        o.shuffle_groups, o.shuffle_seed = 1, int(shuffle_seed)
+    o.staging = int(staging)
+    return o
+
+
+def _scratch(nbytes, dev, stream):
+    """Scratch bytes for kernels enqueued on `stream`: allocated under that stream, so that PyTorch's caching
+    allocator does not hand the block to another stream's tensor while those kernels still use it."""
+    st = stream if stream is not None else torch.cuda.current_stream(dev)
+    with torch.cuda.stream(st):
+        return torch.empty(max(int(nbytes), 8), dtype=torch.uint8, device=dev)
+
+
+def wl_eval_opt_workspace_bytes(n_loops, n_ppl, n_T, n_rho, n_groups, compute, options=None) -> int:
+    return int(_lib.wl_eval_opt_workspace_bytes(n_loops, n_ppl, n_T, n_rho, n_groups, _dtype_code(compute),
+                                                C.byref(options) if options is not None else None))
+
+
 def wl_eval(field, loops, T, rho_cm, phi_cm=None, n_groups=1, compute=torch.float64, W_mean=None,
-            group_sums=None, workspace=None, stream=None, wilson_events=None):
+            group_sums=None, workspace=None, stream=None, wilson_events=None, options=None):
     """Returns (W_mean [n_T][n_rho], group_sums [G][n_T][n_rho]); see include/wl.h.
 
-    wilson_events = (begin, end) torch.cuda.Event pair (enable_timing=True): calls
-    wl_eval_instrumented, which records them around the k_wilson launch."""
+    wilson_events = (begin, end) torch.cuda.Event pair (enable_timing=True): recorded around the k_wilson
+    launch.  options = wl_eval_options(...): calls wl_eval_opt (quadrature order, shuffled groups, staging)."""
     n_loops, n_ppl = _loops_arg(loops)
     T = _cuda_f64(T, "T")
     rho_cm = _cuda_f64(rho_cm, "rho_cm")
@@ -210,18 +261,72 @@ def wl_eval(field, loops, T, rho_cm, phi_cm=None, n_groups=1, compute=torch.floa
     _cuda_f64(group_sums, "group_sums", n_groups * n_T * n_rho)
     cc = _dtype_code(compute)
     if workspace is None:
-        need = int(_lib.wl_eval_workspace_bytes(n_loops, n_ppl, n_T, n_rho, n_groups, cc))
-        workspace = torch.empty(max(need, 8), dtype=torch.uint8, device=dev)
+        workspace = _scratch(wl_eval_opt_workspace_bytes(n_loops, n_ppl, n_T, n_rho, n_groups, cc, options), dev, stream)
     args = (field._h, _ptr(loops), _dtype_code(loops.dtype), n_loops, n_ppl, _ptr(T), n_T,
             _ptr(rho_cm), _ptr(phi_cm), n_rho, int(n_groups), cc, _ptr(W_mean),
             _ptr(group_sums), _ptr(workspace), workspace.numel() * workspace.element_size())
     with torch.cuda.device(dev):
-        if wilson_events is None:
+        if options is not None:
+            if wilson_events is not None:
+                e0, e1 = (_event_handle(ev, stream) for ev in wilson_events)
+                options.event_wilson_begin, options.event_wilson_end = e0, e1
+            _check(_lib.wl_eval_opt(*args, _stream(stream), C.byref(options)), "wl_eval_opt")
+        elif wilson_events is None:
             _check(_lib.wl_eval(*args, _stream(stream)), "wl_eval")
         else:
             e0, e1 = (_event_handle(ev, stream) for ev in wilson_events)
             _check(_lib.wl_eval_instrumented(*args, _stream(stream), e0, e1), "wl_eval_instrumented")
     return W_mean, group_sums
+
+
+def wl_eval_seeded(field, seed, n_loops, n_ppl, T, rho_cm, phi_cm=None, n_groups=1, compute=torch.float64,
+                   storage=torch.float32, loop_begin=0, W_mean=None, group_sums=None, workspace=None, stream=None,
+                   options=None):
+    """wl_eval without an ensemble buffer: loops [loop_begin, loop_begin + n_loops) of ensemble `seed` are
+    regenerated inside the kernel; same bits as wl_loops_generate(storage) + wl_eval.
+    options (quadrature order, shuffled groups) goes through wl_eval_opt with `seeded` set."""
+    T = _cuda_f64(T, "T")
+    rho_cm = _cuda_f64(rho_cm, "rho_cm")
+    n_T, n_rho = T.numel(), rho_cm.numel()
+    phi_cm = _cuda_f64(phi_cm, "phi_cm", n_rho)
+    dev = T.device
+    if W_mean is None:
+        W_mean = torch.empty((n_T, n_rho), dtype=torch.float64, device=dev)
+    if group_sums is None:
+        group_sums = torch.empty((n_groups, n_T, n_rho), dtype=torch.float64, device=dev)
+    cc, sc = _dtype_code(compute), _dtype_code(storage)
+    if options is not None:
+        options.seeded, options.seed, options.loop_begin = 1, int(seed), int(loop_begin)
+    if workspace is None:
+        workspace = _scratch(wl_eval_opt_workspace_bytes(n_loops, n_ppl, n_T, n_rho, n_groups, cc, options), dev, stream)
+    wsb = workspace.numel() * workspace.element_size()
+    with torch.cuda.device(dev):
+        if options is None:
+            _check(_lib.wl_eval_seeded(field._h, int(seed), int(loop_begin), sc, int(n_loops), int(n_ppl), _ptr(T), n_T,
+                                       _ptr(rho_cm), _ptr(phi_cm), n_rho, int(n_groups), cc, _ptr(W_mean),
+                                       _ptr(group_sums), _ptr(workspace), wsb, _stream(stream)), "wl_eval_seeded")
+        else:
+            _check(_lib.wl_eval_opt(field._h, None, sc, int(n_loops), int(n_ppl), _ptr(T), n_T, _ptr(rho_cm),
+                                    _ptr(phi_cm), n_rho, int(n_groups), cc, _ptr(W_mean), _ptr(group_sums),
+                                    _ptr(workspace), wsb, _stream(stream), C.byref(options)), "wl_eval_opt")
+    return W_mean, group_sums
+
+
+def wl_group_permutation(shuffle_seed, n_loops, n_T, device="cuda", stream=None) -> torch.Tensor:
+    """perm [n_T][n_loops] int32: perm[t][i] = pi_t(i), the group membership of shuffle_groups (include/wl.h)."""
+    perm = torch.empty((n_T, n_loops), dtype=torch.int32, device=device)
+    with torch.cuda.device(perm.device):
+        _check(_lib.wl_group_permutation(int(shuffle_seed), int(n_loops), int(n_T), _ptr(perm), _stream(stream)),
+               "wl_group_permutation")
+    return perm
+
+
+def wl_grid_validate(T, rho_cm) -> None:
+    """Host check of grid values (T > 0, rho_cm >= 0, finite); raises WLError(WL_ERR_INVALID_ARG) otherwise."""
+    T = np.ascontiguousarray(T, dtype=np.float64)
+    rho = np.ascontiguousarray(rho_cm, dtype=np.float64)
+    dp = C.POINTER(C.c_double)
+    _check(_lib.wl_grid_validate(T.ctypes.data_as(dp), T.size, rho.ctypes.data_as(dp), rho.size), "wl_grid_validate")
 
 
 def wl_eval_discretization(field, loops, T, rho_cm, phi_cm=None, n_groups=1, compute=torch.float64, stream=None):
@@ -234,7 +339,7 @@ def wl_eval_discretization(field, loops, T, rho_cm, phi_cm=None, n_groups=1, com
     cc = _dtype_code(compute)
     gs3 = torch.empty((3, n_groups, n_T, n_rho), dtype=torch.float64, device=loops.device)
     need = int(_lib.wl_eval_discretization_workspace_bytes(n_loops, n_ppl, n_T, n_rho, n_groups, cc))
-    ws = torch.empty(max(need, 8), dtype=torch.uint8, device=loops.device)
+    ws = _scratch(need, loops.device, stream)
     with torch.cuda.device(loops.device):
         _check(_lib.wl_eval_discretization(field._h, _ptr(loops), _dtype_code(loops.dtype), n_loops, n_ppl, _ptr(T),
                                            n_T, _ptr(rho_cm), _ptr(phi_cm), n_rho, int(n_groups), cc, _ptr(gs3),
@@ -256,21 +361,28 @@ def wl_extrapolate(levels3, want_delta=True, stream=None):
 
 
 def wl_eval_per_loop(field, loops, T, rho_cm, phi_cm=None, compute=torch.float64, want_phase_spin=True,
-                     stream=None):
-    """Per-loop (W, phase, spin), each [n_loops][n_T][n_rho] (phase/spin None if not wanted)."""
-    n_loops, n_ppl = _loops_arg(loops)
+                     stream=None, options=None, n_loops=None, n_ppl=None, storage=torch.float32):
+    """Per-loop (W, phase, spin), each [n_loops][n_T][n_rho] (phase/spin None if not wanted).
+    options: quadrature order / seeded (then loops may be None and n_loops, n_ppl, storage say what to generate)."""
+    if loops is None:
+        if options is None or not options.seeded:
+            raise ValueError("loops=None needs seeded options")
+    else:
+        n_loops, n_ppl = _loops_arg(loops)
     T = _cuda_f64(T, "T")
     rho_cm = _cuda_f64(rho_cm, "rho_cm")
     n_T, n_rho = T.numel(), rho_cm.numel()
     phi_cm = _cuda_f64(phi_cm, "phi_cm", n_rho)
-    dev = loops.device
+    dev = T.device
     W = torch.empty((n_loops, n_T, n_rho), dtype=torch.float64, device=dev)
     ph = torch.empty_like(W) if want_phase_spin else None
     sp = torch.empty_like(W) if want_phase_spin else None
+    ldt = _dtype_code(loops.dtype if loops is not None else storage)
     with torch.cuda.device(dev):
-        _check(_lib.wl_eval_per_loop(field._h, _ptr(loops), _dtype_code(loops.dtype), n_loops, n_ppl, _ptr(T),
-                                     n_T, _ptr(rho_cm), _ptr(phi_cm), n_rho, _dtype_code(compute), _ptr(W),
-                                     _ptr(ph), _ptr(sp), _stream(stream)), "wl_eval_per_loop")
+        _check(_lib.wl_eval_per_loop_opt(field._h, _ptr(loops), ldt, int(n_loops), int(n_ppl), _ptr(T),
+                                         n_T, _ptr(rho_cm), _ptr(phi_cm), n_rho, _dtype_code(compute), _ptr(W),
+                                         _ptr(ph), _ptr(sp), _stream(stream),
+                                         C.byref(options) if options is not None else None), "wl_eval_per_loop_opt")
     return W, ph, sp
 
 

@@ -14,10 +14,68 @@ bool sizes_ok(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups)
     if (n_loops % n_groups != 0) return false;                       // equal groups
     if ((int64_t)n_T * n_rho > (1 << 24)) return false;
     if (n_loops > (1LL << 40)) return false;
+    // launch limits, checked before anything is enqueued: k_wilson has at most n_loops x tiles(128 points)
+    // CTAs, the group reductions n_groups x tiles(256 points)
+    const int64_t n_grid = (int64_t)n_T * n_rho;
+    if (n_loops * ((n_grid + 127) / 128) > 0x7fffffffLL) return false;
+    if ((int64_t)n_groups * ((n_grid + 255) / 256) > 0x7fffffffLL) return false;
     return true;
 }
 
 bool dtype_ok(wl_dtype d) { return d == WL_F32 || d == WL_F64; }
+
+bool seeded_ppl_ok(int n_ppl) { return n_ppl >= 2 && n_ppl <= kMaxPplSeeded && (n_ppl & (n_ppl - 1)) == 0; }
+
+// Options as the launches see them; false on an invalid option block.
+struct Opt {
+    int quad = 1, seeded = 0, shuffle = 0, bulk = 0;
+    uint64_t seed = 0, shuffle_seed = 0;
+    int64_t loop_begin = 0;
+    void* ev0 = nullptr;
+    void* ev1 = nullptr;
+};
+
+bool read_options(const wl_eval_options* o, int n_ppl, int64_t n_loops, Opt* out)
+{
+    if (!o) return true;
+    if (o->struct_size != sizeof(wl_eval_options)) return false;
+    if (o->quadrature_order < 0 || o->quadrature_order > 3) return false;
+    out->quad = o->quadrature_order == 0 ? 1 : o->quadrature_order;
+    out->seeded = o->seeded != 0;
+    out->seed = o->seed;
+    out->loop_begin = o->loop_begin;
+    if (out->seeded && (!seeded_ppl_ok(n_ppl) || o->loop_begin < 0)) return false;
+    out->shuffle = o->shuffle_groups != 0;
+    out->shuffle_seed = o->shuffle_seed;
+    if (out->shuffle && n_loops > 0x7fffffffLL) return false;
+    if (o->staging != 0 && o->staging != 1) return false;
+    out->bulk = o->staging;
+    out->ev0 = o->event_wilson_begin;
+    out->ev1 = o->event_wilson_end;
+    return true;
+}
+
+EvalArgs make_args(const wl_field* field, const void* d_loops, wl_dtype loop_dtype, int64_t n_loops, int n_ppl,
+                   const double* d_T, int n_T, const double* d_rho_cm, const double* d_phi_cm, int n_rho,
+                   const Opt& o)
+{
+    EvalArgs a;
+    a.loops = d_loops; a.loops_are_f64 = (loop_dtype == WL_F64); a.n_loops = n_loops; a.n_ppl = n_ppl;
+    a.T = d_T; a.rho = d_rho_cm; a.phi = d_phi_cm; a.n_T = n_T; a.n_rho = n_rho;
+    a.p0 = field->p0; a.p1 = field->p1; a.scalar = field->scalar; a.disc = 0;
+    a.quad = o.quad; a.seeded = o.seeded; a.bulk = o.bulk; a.seed = o.seed; a.loop_begin = o.loop_begin;
+    a.partial = nullptr; a.phase_out = nullptr; a.spin_out = nullptr;
+    return a;
+}
+
+size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
+
+wl_status launch_status(cudaError_t e)
+{
+    if (e == cudaSuccess) return WL_OK;
+    cudaGetLastError();
+    return e == cudaErrorInvalidValue ? WL_ERR_UNSUPPORTED : WL_ERR_CUDA;
+}
 
 }  // namespace
 
@@ -55,23 +113,50 @@ wl_status wl_field_create_particle(wl_profile profile, const double* h_params, i
 
 void wl_field_destroy(wl_field* field) { delete field; }
 
+wl_status wl_grid_validate(const double* h_T, int n_T, const double* h_rho_cm, int n_rho)
+{
+    if (!h_T || !h_rho_cm || n_T < 1 || n_rho < 1) return WL_ERR_INVALID_ARG;
+    for (int k = 0; k < n_T; ++k)
+        if (!std::isfinite(h_T[k]) || !(h_T[k] > 0.0)) return WL_ERR_INVALID_ARG;
+    for (int k = 0; k < n_rho; ++k)
+        if (!std::isfinite(h_rho_cm[k]) || !(h_rho_cm[k] >= 0.0)) return WL_ERR_INVALID_ARG;
+    return WL_OK;
+}
+
 wl_status wl_loops_generate(void* d_loops, wl_dtype storage, int64_t loop_begin, int64_t n_loops, int n_ppl,
                             uint64_t seed, void* stream)
 {
     if (!dtype_ok(storage) || n_loops < 0 || loop_begin < 0) return WL_ERR_INVALID_ARG;
-    if (n_ppl < 2 || n_ppl > kMaxPpl || (n_ppl & (n_ppl - 1)) != 0) return WL_ERR_INVALID_ARG;
+    if (!seeded_ppl_ok(n_ppl)) return WL_ERR_INVALID_ARG;
     if (n_loops == 0) return WL_OK;
     if (!d_loops) return WL_ERR_INVALID_ARG;
-    cudaError_t e = launch_generate(d_loops, storage == WL_F64, loop_begin, n_loops, n_ppl, seed,
-                                    (cudaStream_t)stream);
-    return e == cudaSuccess ? WL_OK : WL_ERR_CUDA;
+    return launch_status(launch_generate(d_loops, storage == WL_F64, loop_begin, n_loops, n_ppl, seed,
+                                         (cudaStream_t)stream));
+}
+
+void wl_eval_options_default(wl_eval_options* opt)
+{
+    if (!opt) return;
+    *opt = wl_eval_options();
+    opt->struct_size = sizeof(wl_eval_options);
+    opt->quadrature_order = 1;
 }
 
 size_t wl_eval_workspace_bytes(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups, wl_dtype compute)
 {
+    return wl_eval_opt_workspace_bytes(n_loops, n_ppl, n_T, n_rho, n_groups, compute, nullptr);
+}
+
+size_t wl_eval_opt_workspace_bytes(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups, wl_dtype compute,
+                                   const wl_eval_options* opt)
+{
     if (!sizes_ok(n_loops, n_ppl, n_T, n_rho, n_groups) || !dtype_ok(compute)) return 0;
-    const EvalPlan p = make_eval_plan(n_loops, n_ppl, n_T, n_rho, n_groups, compute, false);
-    return (size_t)p.n_units * (size_t)p.n_grid * sizeof(double);
+    Opt o;
+    if (!read_options(opt, n_ppl, n_loops, &o)) return 0;
+    const EvalPlan p = make_eval_plan(n_loops, n_ppl, n_T, n_rho, n_groups, compute, o.shuffle != 0);
+    const size_t partial = (size_t)p.n_units * (size_t)p.n_grid * sizeof(double);
+    if (!o.shuffle) return partial;
+    return align256(partial) + align256((size_t)n_T * (size_t)n_loops * sizeof(int32_t));   // W per loop, membership table
 }
 
 int wl_eval_launch_count(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups, wl_dtype compute)
@@ -85,9 +170,8 @@ wl_status wl_eval(const wl_field* field, const void* d_loops, wl_dtype loop_dtyp
                   int n_groups, wl_dtype compute, double* d_W_mean, double* d_group_sums,
                   void* d_workspace, size_t workspace_bytes, void* stream)
 {
-    return wl_eval_instrumented(field, d_loops, loop_dtype, n_loops, n_ppl, d_T, n_T, d_rho_cm, d_phi_cm, n_rho,
-                                n_groups, compute, d_W_mean, d_group_sums, d_workspace, workspace_bytes, stream,
-                                nullptr, nullptr);
+    return wl_eval_opt(field, d_loops, loop_dtype, n_loops, n_ppl, d_T, n_T, d_rho_cm, d_phi_cm, n_rho, n_groups,
+                       compute, d_W_mean, d_group_sums, d_workspace, workspace_bytes, stream, nullptr);
 }
 
 wl_status wl_eval_instrumented(const wl_field* field, const void* d_loops, wl_dtype loop_dtype, int64_t n_loops,
@@ -97,27 +181,67 @@ wl_status wl_eval_instrumented(const wl_field* field, const void* d_loops, wl_dt
                                size_t workspace_bytes, void* stream, void* event_wilson_begin,
                                void* event_wilson_end)
 {
-    if (!field || !d_loops || !d_T || !d_rho_cm || !d_W_mean || !d_group_sums) return WL_ERR_INVALID_ARG;
+    wl_eval_options opt;
+    wl_eval_options_default(&opt);
+    opt.event_wilson_begin = event_wilson_begin;
+    opt.event_wilson_end = event_wilson_end;
+    return wl_eval_opt(field, d_loops, loop_dtype, n_loops, n_ppl, d_T, n_T, d_rho_cm, d_phi_cm, n_rho, n_groups,
+                       compute, d_W_mean, d_group_sums, d_workspace, workspace_bytes, stream, &opt);
+}
+
+wl_status wl_eval_seeded(const wl_field* field, uint64_t seed, int64_t loop_begin, wl_dtype storage,
+                         int64_t n_loops, int n_ppl, const double* d_T, int n_T, const double* d_rho_cm,
+                         const double* d_phi_cm, int n_rho, int n_groups, wl_dtype compute, double* d_W_mean,
+                         double* d_group_sums, void* d_workspace, size_t workspace_bytes, void* stream)
+{
+    wl_eval_options opt;
+    wl_eval_options_default(&opt);
+    opt.seeded = 1;
+    opt.seed = seed;
+    opt.loop_begin = loop_begin;
+    return wl_eval_opt(field, nullptr, storage, n_loops, n_ppl, d_T, n_T, d_rho_cm, d_phi_cm, n_rho, n_groups,
+                       compute, d_W_mean, d_group_sums, d_workspace, workspace_bytes, stream, &opt);
+}
+
+wl_status wl_eval_opt(const wl_field* field, const void* d_loops, wl_dtype loop_dtype, int64_t n_loops, int n_ppl,
+                      const double* d_T, int n_T, const double* d_rho_cm, const double* d_phi_cm, int n_rho,
+                      int n_groups, wl_dtype compute, double* d_W_mean, double* d_group_sums,
+                      void* d_workspace, size_t workspace_bytes, void* stream, const wl_eval_options* opt)
+{
+    if (!field || !d_T || !d_rho_cm || !d_W_mean || !d_group_sums) return WL_ERR_INVALID_ARG;
     if (!dtype_ok(loop_dtype) || !dtype_ok(compute)) return WL_ERR_INVALID_ARG;
     if (!sizes_ok(n_loops, n_ppl, n_T, n_rho, n_groups)) return WL_ERR_INVALID_ARG;
-    const EvalPlan plan = make_eval_plan(n_loops, n_ppl, n_T, n_rho, n_groups, compute, false);
-    const size_t need = (size_t)plan.n_units * (size_t)plan.n_grid * sizeof(double);
+    Opt o;
+    if (!read_options(opt, n_ppl, n_loops, &o)) return WL_ERR_INVALID_ARG;
+    if (!o.seeded && !d_loops) return WL_ERR_INVALID_ARG;
+    const size_t need = wl_eval_opt_workspace_bytes(n_loops, n_ppl, n_T, n_rho, n_groups, compute, opt);
     if (!d_workspace || workspace_bytes < need) return WL_ERR_WORKSPACE;
+    const EvalPlan plan = make_eval_plan(n_loops, n_ppl, n_T, n_rho, n_groups, compute, o.shuffle != 0);
 
-    EvalArgs a;
-    a.loops = d_loops; a.loops_are_f64 = (loop_dtype == WL_F64); a.n_loops = n_loops; a.n_ppl = n_ppl;
-    a.T = d_T; a.rho = d_rho_cm; a.phi = d_phi_cm; a.n_T = n_T; a.n_rho = n_rho;
-    a.p0 = field->p0; a.p1 = field->p1; a.scalar = field->scalar; a.disc = 0;
+    EvalArgs a = make_args(field, d_loops, loop_dtype, n_loops, n_ppl, d_T, n_T, d_rho_cm, d_phi_cm, n_rho, o);
     a.partial = reinterpret_cast<double*>(d_workspace);
-    a.phase_out = nullptr; a.spin_out = nullptr;
     cudaStream_t s = (cudaStream_t)stream;
-    if (event_wilson_begin && cudaEventRecord((cudaEvent_t)event_wilson_begin, s) != cudaSuccess) return WL_ERR_CUDA;
+    if (o.ev0 && cudaEventRecord((cudaEvent_t)o.ev0, s) != cudaSuccess) return launch_status(cudaErrorUnknown);
     cudaError_t e = launch_wilson(plan, a, field->profile, compute, s);
-    if (e != cudaSuccess) return e == cudaErrorInvalidValue ? WL_ERR_UNSUPPORTED : WL_ERR_CUDA;
-    if (event_wilson_end && cudaEventRecord((cudaEvent_t)event_wilson_end, s) != cudaSuccess) return WL_ERR_CUDA;
-    e = launch_group_reduce(a.partial, plan.n_units, plan.units_per_group, n_groups, plan.n_grid, n_loops,
-                            d_group_sums, d_W_mean, s);
-    return e == cudaSuccess ? WL_OK : WL_ERR_CUDA;
+    if (e != cudaSuccess) return launch_status(e);
+    if (o.ev1 && cudaEventRecord((cudaEvent_t)o.ev1, s) != cudaSuccess) return launch_status(cudaErrorUnknown);
+    if (!o.shuffle)
+        return launch_status(launch_group_reduce(a.partial, plan.units_per_group, n_groups, plan.n_grid, n_loops,
+                                                 d_group_sums, d_W_mean, s));
+    // shuffled groups: the workspace holds W per loop, then the membership table
+    int32_t* perm = reinterpret_cast<int32_t*>(reinterpret_cast<unsigned char*>(d_workspace)
+                                               + align256((size_t)n_loops * plan.n_grid * sizeof(double)));
+    e = launch_group_permutation(o.shuffle_seed, n_loops, n_T, perm, s);
+    if (e != cudaSuccess) return launch_status(e);
+    return launch_status(launch_group_reduce_shuffled(a.partial, perm, n_loops, n_T, n_rho, n_groups, d_group_sums,
+                                                      d_W_mean, s));
+}
+
+wl_status wl_group_permutation(uint64_t shuffle_seed, int64_t n_loops, int n_T, int32_t* d_perm, void* stream)
+{
+    if (!d_perm || n_loops < 1 || n_loops > 0x7fffffffLL || n_T < 1) return WL_ERR_INVALID_ARG;
+    if ((n_loops * n_T + 255) / 256 > 0x7fffffffLL) return WL_ERR_INVALID_ARG;
+    return launch_status(launch_group_permutation(shuffle_seed, n_loops, n_T, d_perm, (cudaStream_t)stream));
 }
 
 namespace {
@@ -156,19 +280,16 @@ wl_status wl_eval_discretization(const wl_field* field, const void* d_loops, wl_
     const size_t level = (size_t)plan.n_units * (size_t)plan.n_grid;
     if (!d_workspace || workspace_bytes < 3 * level * sizeof(double)) return WL_ERR_WORKSPACE;
 
-    EvalArgs a;
-    a.loops = d_loops; a.loops_are_f64 = (loop_dtype == WL_F64); a.n_loops = n_loops; a.n_ppl = n_ppl;
-    a.T = d_T; a.rho = d_rho_cm; a.phi = d_phi_cm; a.n_T = n_T; a.n_rho = n_rho;
-    a.p0 = field->p0; a.p1 = field->p1; a.scalar = field->scalar; a.disc = 1;
+    EvalArgs a = make_args(field, d_loops, loop_dtype, n_loops, n_ppl, d_T, n_T, d_rho_cm, d_phi_cm, n_rho, Opt());
+    a.disc = 1;
     a.partial = reinterpret_cast<double*>(d_workspace);
-    a.phase_out = nullptr; a.spin_out = nullptr;
     cudaStream_t s = (cudaStream_t)stream;
     cudaError_t e = launch_wilson(plan, a, field->profile, compute, s);
-    if (e != cudaSuccess) return e == cudaErrorInvalidValue ? WL_ERR_UNSUPPORTED : WL_ERR_CUDA;
+    if (e != cudaSuccess) return launch_status(e);
     for (int lev = 0; lev < 3; ++lev) {
-        e = launch_group_reduce(a.partial + lev * level, plan.n_units, plan.units_per_group, n_groups, plan.n_grid,
+        e = launch_group_reduce(a.partial + lev * level, plan.units_per_group, n_groups, plan.n_grid,
                                 n_loops, d_group_sums3 + (size_t)lev * n_groups * plan.n_grid, nullptr, s);
-        if (e != cudaSuccess) return WL_ERR_CUDA;
+        if (e != cudaSuccess) return launch_status(e);
     }
     return WL_OK;
 }
@@ -176,8 +297,7 @@ wl_status wl_eval_discretization(const wl_field* field, const void* d_loops, wl_
 wl_status wl_extrapolate(const double* d_levels3, int64_t n, double* d_W_inf, double* d_delta, void* stream)
 {
     if (!d_levels3 || !d_W_inf || n < 1) return WL_ERR_INVALID_ARG;
-    cudaError_t e = launch_extrapolate(d_levels3, n, d_W_inf, d_delta, (cudaStream_t)stream);
-    return e == cudaSuccess ? WL_OK : WL_ERR_CUDA;
+    return launch_status(launch_extrapolate(d_levels3, n, d_W_inf, d_delta, (cudaStream_t)stream));
 }
 
 wl_status wl_eval_per_loop(const wl_field* field, const void* d_loops, wl_dtype loop_dtype, int64_t n_loops,
@@ -185,18 +305,26 @@ wl_status wl_eval_per_loop(const wl_field* field, const void* d_loops, wl_dtype 
                            const double* d_phi_cm, int n_rho, wl_dtype compute,
                            double* d_W, double* d_phase, double* d_spin, void* stream)
 {
-    if (!field || !d_loops || !d_T || !d_rho_cm || !d_W) return WL_ERR_INVALID_ARG;
+    return wl_eval_per_loop_opt(field, d_loops, loop_dtype, n_loops, n_ppl, d_T, n_T, d_rho_cm, d_phi_cm, n_rho,
+                                compute, d_W, d_phase, d_spin, stream, nullptr);
+}
+
+wl_status wl_eval_per_loop_opt(const wl_field* field, const void* d_loops, wl_dtype loop_dtype, int64_t n_loops,
+                               int n_ppl, const double* d_T, int n_T, const double* d_rho_cm,
+                               const double* d_phi_cm, int n_rho, wl_dtype compute,
+                               double* d_W, double* d_phase, double* d_spin, void* stream,
+                               const wl_eval_options* opt)
+{
+    if (!field || !d_T || !d_rho_cm || !d_W) return WL_ERR_INVALID_ARG;
     if (!dtype_ok(loop_dtype) || !dtype_ok(compute)) return WL_ERR_INVALID_ARG;
     if (!sizes_ok(n_loops, n_ppl, n_T, n_rho, 1)) return WL_ERR_INVALID_ARG;
+    Opt o;
+    if (!read_options(opt, n_ppl, 1, &o)) return WL_ERR_INVALID_ARG;
+    if (!o.seeded && !d_loops) return WL_ERR_INVALID_ARG;
     const EvalPlan plan = make_eval_plan(n_loops, n_ppl, n_T, n_rho, 1, compute, true);
-    EvalArgs a;
-    a.loops = d_loops; a.loops_are_f64 = (loop_dtype == WL_F64); a.n_loops = n_loops; a.n_ppl = n_ppl;
-    a.T = d_T; a.rho = d_rho_cm; a.phi = d_phi_cm; a.n_T = n_T; a.n_rho = n_rho;
-    a.p0 = field->p0; a.p1 = field->p1; a.scalar = field->scalar; a.disc = 0;
+    EvalArgs a = make_args(field, d_loops, loop_dtype, n_loops, n_ppl, d_T, n_T, d_rho_cm, d_phi_cm, n_rho, o);
     a.partial = d_W; a.phase_out = d_phase; a.spin_out = d_spin;
-    cudaError_t e = launch_wilson(plan, a, field->profile, compute, (cudaStream_t)stream);
-    if (e != cudaSuccess) return e == cudaErrorInvalidValue ? WL_ERR_UNSUPPORTED : WL_ERR_CUDA;
-    return WL_OK;
+    return launch_status(launch_wilson(plan, a, field->profile, compute, (cudaStream_t)stream));
 }
 
 wl_status wl_jackknife_finalize(const double* d_group_sums, int n_groups, int64_t n_loops, int n_T, int n_rho,
@@ -205,9 +333,8 @@ wl_status wl_jackknife_finalize(const double* d_group_sums, int n_groups, int64_
     if (!d_group_sums || !d_mean || !d_err) return WL_ERR_INVALID_ARG;
     if (n_groups < 2 || n_loops < 1 || n_loops % n_groups != 0 || n_T < 1 || n_rho < 1) return WL_ERR_INVALID_ARG;
     if ((int64_t)n_T * n_rho > (1 << 24)) return WL_ERR_INVALID_ARG;
-    cudaError_t e = launch_finalize(d_group_sums, n_groups, n_loops, n_T * n_rho, d_mean, d_err, d_delete_one,
-                                    (cudaStream_t)stream);
-    return e == cudaSuccess ? WL_OK : WL_ERR_CUDA;
+    return launch_status(launch_finalize(d_group_sums, n_groups, n_loops, n_T * n_rho, d_mean, d_err, d_delete_one,
+                                         (cudaStream_t)stream));
 }
 
 const char* wl_status_string(wl_status status)
@@ -222,6 +349,6 @@ const char* wl_status_string(wl_status status)
     return "unknown status";
 }
 
-const char* wl_version(void) { return "1.0"; }
+const char* wl_version(void) { return "2.0"; }
 
 }  // extern "C"

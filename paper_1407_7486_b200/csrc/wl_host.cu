@@ -12,6 +12,30 @@ namespace {
 cudaMemPool_t g_pool[64] = {};
 std::mutex g_pool_mutex;
 
+// The two streams (compute, copy) and two events of a call are created once per device and kept, like the
+// pool; g_call_mutex serialises wl_eval_host calls (they share these handles).
+struct HostHandles {
+    cudaStream_t s = nullptr, copy = nullptr;
+    cudaEvent_t ev[2] = {nullptr, nullptr};
+};
+HostHandles g_handles[64];
+std::mutex g_call_mutex;
+
+cudaError_t host_handles(HostHandles** out)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    HostHandles& h = g_handles[dev];
+    if (!h.s && (e = cudaStreamCreateWithFlags(&h.s, cudaStreamNonBlocking)) != cudaSuccess) return e;
+    if (!h.copy && (e = cudaStreamCreateWithFlags(&h.copy, cudaStreamNonBlocking)) != cudaSuccess) return e;
+    for (cudaEvent_t& ev : h.ev)
+        if (!ev && (e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming)) != cudaSuccess) return e;
+    *out = &h;
+    return cudaSuccess;
+}
+
 cudaError_t host_pool(cudaMemPool_t* out)
 {
     std::lock_guard<std::mutex> lock(g_pool_mutex);
@@ -44,12 +68,10 @@ struct DeviceBuffers {
     ~DeviceBuffers()
     {
         if (s) {
+            if (copy) cudaStreamSynchronize(copy);   // a copy may still be writing into a buffer (early error return)
             for (void* q : p) if (q) cudaFreeAsync(q, s);
             cudaStreamSynchronize(s);
         }
-        for (cudaEvent_t e : ev) if (e) cudaEventDestroy(e);
-        if (s) cudaStreamDestroy(s);
-        if (copy) cudaStreamDestroy(copy);
     }
 };
 
@@ -82,9 +104,10 @@ extern "C" wl_status wl_eval_host(const wl_field* field, const void* h_loops, wl
     DeviceBuffers d;
     enum { LOOPS, T, RHO, PHI, MEAN, GS, ERR, WS };
 #define WL_TRY(call) do { if ((call) != cudaSuccess) { cudaGetLastError(); return WL_ERR_CUDA; } } while (0)
-    WL_TRY(cudaStreamCreateWithFlags(&d.s, cudaStreamNonBlocking));
-    WL_TRY(cudaStreamCreateWithFlags(&d.copy, cudaStreamNonBlocking));
-    for (cudaEvent_t& e : d.ev) WL_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    std::lock_guard<std::mutex> call_lock(g_call_mutex);
+    HostHandles* hh = nullptr;
+    WL_TRY(host_handles(&hh));
+    d.s = hh->s; d.copy = hh->copy; d.ev[0] = hh->ev[0]; d.ev[1] = hh->ev[1];
     cudaMemPool_t pool;
     WL_TRY(host_pool(&pool));
 #define WL_ALLOC(slot, bytes) WL_TRY(cudaMallocFromPoolAsync(&d.p[slot], (bytes), pool, d.s))
@@ -132,12 +155,13 @@ extern "C" wl_status wl_eval_host(const wl_field* field, const void* h_loops, wl
         a.T = reinterpret_cast<const double*>(d.p[T]); a.rho = reinterpret_cast<const double*>(d.p[RHO]);
         a.phi = reinterpret_cast<const double*>(d.p[PHI]); a.n_T = n_T; a.n_rho = n_rho;
         a.p0 = field->p0; a.p1 = field->p1; a.scalar = field->scalar; a.disc = 0;
+        a.quad = 1; a.seeded = 0; a.bulk = 0; a.seed = 0; a.loop_begin = 0;
         a.partial = partial + (size_t)(l0 / plan.loops_per_unit) * plan.n_grid;
         a.phase_out = nullptr; a.spin_out = nullptr;
         cudaError_t e = wl::launch_wilson(sub, a, field->profile, compute, d.s);
         if (e != cudaSuccess) { cudaGetLastError(); return e == cudaErrorInvalidValue ? WL_ERR_UNSUPPORTED : WL_ERR_CUDA; }
     }
-    if (wl::launch_group_reduce(partial, plan.n_units, plan.units_per_group, n_groups, plan.n_grid, n_loops,
+    if (wl::launch_group_reduce(partial, plan.units_per_group, n_groups, plan.n_grid, n_loops,
                                 reinterpret_cast<double*>(d.p[GS]), mean, d.s) != cudaSuccess) {
         cudaGetLastError();
         return WL_ERR_CUDA;

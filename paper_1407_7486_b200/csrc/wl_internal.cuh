@@ -16,7 +16,7 @@ struct wl_field {
 
 namespace wl {
 
-constexpr int kMaxPpl = 8192;        // generator limit (one loop in shared memory as double2)
+constexpr int kMaxPplSeeded = 1 << 16;   // generator / seeded-evaluation limit on N (skeleton of <= 128 points)
 
 // ---- how wl_eval cuts the work (a function of the sizes only, never of the device) ----
 struct EvalPlan {
@@ -26,16 +26,15 @@ struct EvalPlan {
     int n_tiles;         // CTAs along the grid: ceil(n_grid / (threads * P))
     int loops_per_unit;  // consecutive loops one CTA sums before writing a partial
     int64_t n_units;     // n_loops / loops_per_unit
-    int units_per_group; // (n_loops / n_groups) / loops_per_unit
-    int chunk_points;    // loop points staged in shared memory at a time
+    int64_t units_per_group; // (n_loops / n_groups) / loops_per_unit
 };
 
 EvalPlan make_eval_plan(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups, wl_dtype compute,
                         bool per_loop);
 
 struct EvalArgs {
-    const void* loops;          // [n_loops][n_ppl][2]
-    int loops_are_f64;
+    const void* loops;          // [n_loops][n_ppl][2]; unused when seeded
+    int loops_are_f64;          // storage precision of the loop coordinates (also the rounding a seeded run emulates)
     int64_t n_loops;
     int n_ppl;
     const double* T;            // [n_T]
@@ -44,7 +43,12 @@ struct EvalArgs {
     int n_T, n_rho;
     double p0, p1;              // field parameters
     int scalar;                 // W = cos(phase) only
-    int disc;                   // discretisation estimate (three levels, generic kernel only)
+    int disc;                   // discretisation estimate (three levels)
+    int quad;                   // Gauss-Legendre points in t for eq. (24): 1 (midpoint), 2, 3
+    int seeded;                 // 1: regenerate every loop from (seed, loop_begin + loop) instead of reading `loops`
+    int bulk;                   // 1: stage raw chunks by cp.async.bulk + mbarrier (measurement variant)
+    uint64_t seed;
+    int64_t loop_begin;
     double* partial;            // [n_units][n_grid]
     double* phase_out;          // per-loop mode only, nullable
     double* spin_out;           // per-loop mode only, nullable
@@ -52,15 +56,22 @@ struct EvalArgs {
 
 cudaError_t launch_wilson(const EvalPlan& plan, const EvalArgs& a, int profile, wl_dtype compute,
                           cudaStream_t s);
-// FP32, sech^2, phi_cm == NULL: the packed-FP32 kernel of wl_wilson_sech2_f32.cu (plan.P >= 2).
+// FP32, sech^2: the packed-FP32 kernels of wl_wilson_sech2_f32.cu.
 cudaError_t launch_wilson_sech2_f32(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s);
-// FP32, flux tube (eq. (68)), phi_cm == NULL: the packed-FP32 kernel of wl_wilson_fluxtube_f32.cu (plan.P >= 2).
+// FP32, flux tube (eq. (68)): the packed-FP32 kernels of wl_wilson_fluxtube_f32.cu.
 cudaError_t launch_wilson_fluxtube_f32(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s);
-// FP64, sech^2, phi_cm == NULL: the lean FP64 kernel of wl_wilson_sech2_f64.cu (plan.P = 1 or 2).
+// FP64, sech^2: the lean FP64 kernels of wl_wilson_sech2_f64.cu (plan.P = 1 or 2).
 cudaError_t launch_wilson_sech2_f64(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s);
-cudaError_t launch_group_reduce(const double* partial, int64_t n_units, int units_per_group, int n_groups,
+// Is (quadrature order, phi_cm, discretisation, staging) a combination the lean kernels are instantiated for?
+bool lean_combination(const EvalArgs& a);
+
+cudaError_t launch_group_reduce(const double* partial, int64_t units_per_group, int n_groups,
                                 int n_grid, int64_t n_loops, double* group_sums, double* W_mean,
                                 cudaStream_t s);
+cudaError_t launch_group_permutation(uint64_t seed, int64_t n_loops, int n_T, int32_t* perm, cudaStream_t s);
+cudaError_t launch_group_reduce_shuffled(const double* W_loop, const int32_t* perm, int64_t n_loops, int n_T,
+                                         int n_rho, int n_groups, double* group_sums, double* W_mean,
+                                         cudaStream_t s);
 cudaError_t launch_finalize(const double* group_sums, int n_groups, int64_t n_loops, int n_grid,
                             double* mean, double* err, double* delete_one, cudaStream_t s);
 cudaError_t launch_extrapolate(const double* levels3, int64_t n, double* W_inf, double* delta, cudaStream_t s);

@@ -106,7 +106,7 @@ def test_compute_calls_reject_bad_arguments_without_a_gpu(lib):
     lib.wl_loops_generate.argtypes = [vp, C.c_int, C.c_int64, C.c_int64, C.c_int, C.c_uint64, vp]
     dummy = C.c_void_p(16)
     assert lib.wl_loops_generate(dummy, 1, 0, 4, 100, 1, None) == 1      # not a power of two
-    assert lib.wl_loops_generate(dummy, 1, 0, 4, 16384, 1, None) == 1    # above the generator limit
+    assert lib.wl_loops_generate(dummy, 1, 0, 4, 131072, 1, None) == 1   # above the generator limit (65536)
     assert lib.wl_loops_generate(dummy, 1, 0, -1, 64, 1, None) == 1
     assert lib.wl_loops_generate(dummy, 1, 0, 0, 64, 1, None) == 0       # empty: no-op
     lib.wl_jackknife_finalize.restype = C.c_int
