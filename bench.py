@@ -36,16 +36,23 @@ METRIC = "wilson_loop_point_evals_per_s"
 UNIT = "point-evals/s"
 
 # algorithmic work per point-eval of the sech^2 profile in FP32
-# (SURVEY.md section 8(d)): 29 plain FP32 lane-ops + 7 special-function lane-ops.
+# (SURVEY.md section 8(d)): 29 plain FP32 lane-ops + 7 special-function lane-ops at the midpoint rule; every
+# further Gauss-Legendre node of eq. (24) adds one segment evaluation (21 plain + 4 special-function).
 ALG_PLAIN_OPS = 29
 ALG_SFU_OPS = 7
+ALG_NODE_PLAIN_OPS = 21
+ALG_NODE_SFU_OPS = 4
 ALG_OPS_UNIFORM = 4
-ALG_F64_OPS_SECH2 = 97            # FP64-pipe lane-ops per point-eval, branch-free formulation
+ALG_OPS_FLUXTUBE = 16             # 14 plain + 2 reciprocals
+# FP64 has no special-function unit: the seven elementary functions are counted as their shortest double-precision
+# sequences (2 x sqrt/rsqrt: 9, 2 x 2^x: 13, 2 x reciprocal: 4, log2(1+E): 20 -> 72) + the 29 plain ops.
+ALG_F64_OPS_SECH2 = 101
+KERNEL_F64_OPS_SECH2 = 97         # what k_wilson<Sech2LeanF64> issues on the FP64 pipe (one shared reciprocal)
 SM_COUNT = 148
 ISSUE_LANES_PER_CLK_SM = 128      # 4 sub-partitions x 1 warp instruction (32 lanes) per clock
 FP64_LANES_PER_CLK_SM = 64        # measured 63.8 (profiles/r01_pipe_rates.md)
 SFU_LANES_PER_CLK_SM = 16         # measured 15.9
-KERNEL_SFU_OPS = 5                # MUFU per point-eval in k_wilson_sech2_f32 (sqrt, rsqrt, 2 x ex2, rcp)
+KERNEL_SFU_OPS = 5                # MUFU per point-eval in k_wilson<Sech2PackedF32> at Q = 1 (sqrt, rsqrt, 2 x ex2, rcp); + 2 per extra node
 
 
 def affinity_cores():
@@ -212,8 +219,17 @@ def run_ours(args, cfg):
     field = api.wl_field_create(cfg.profile, cfg.params)
     sh = shard.shard_groups(cfg.n_loops * world, cfg.n_groups * world, world, rank)
     tdt = torch.float32 if cfg.loop_dtype == "f32" else torch.float64
-    loops = api.wl_loops_generate(sh.n_loops, cfg.n_ppl, cfg.seed, tdt, loop_begin=sh.loop_begin)
-    ws_bytes = api.wl_eval_workspace_bytes(sh.n_loops, cfg.n_ppl, cfg.n_T, cfg.n_rho, sh.n_groups, compute)
+    seeded = args.loops == "seeded"
+    loops = None if seeded else api.wl_loops_generate(sh.n_loops, cfg.n_ppl, cfg.seed, tdt, loop_begin=sh.loop_begin)
+    loop_bytes = sh.n_loops * cfg.n_ppl * 2 * (4 if cfg.loop_dtype == "f32" else 8)
+
+    def options():
+        if args.quadrature == 1 and not args.shuffle and args.staging == "default" and not seeded:
+            return None
+        return api.wl_eval_options(quadrature_order=args.quadrature, shuffle_seed=(cfg.seed + 1000 if args.shuffle else None),
+                                   staging=(1 if args.staging == "bulk" else 0),
+                                   seed=(cfg.seed if seeded else None), loop_begin=sh.loop_begin)
+    ws_bytes = api.wl_eval_opt_workspace_bytes(sh.n_loops, cfg.n_ppl, cfg.n_T, cfg.n_rho, sh.n_groups, compute, options())
     workspace = torch.empty(max(ws_bytes, 8), dtype=torch.uint8, device="cuda")
     W_mean = torch.empty((cfg.n_T, cfg.n_rho), dtype=torch.float64, device="cuda")
     gs_local = torch.empty((sh.n_groups, cfg.n_T, cfg.n_rho), dtype=torch.float64, device="cuda")
@@ -221,8 +237,16 @@ def run_ours(args, cfg):
     stream = torch.cuda.current_stream()
 
     def step(events=None):
-        api.wl_eval(field, loops, Td, rd, pd, n_groups=sh.n_groups, compute=compute, W_mean=W_mean,
-                    group_sums=gs_local, workspace=workspace, wilson_events=events)
+        if seeded:
+            opt = options()
+            if events is not None:
+                opt.event_wilson_begin, opt.event_wilson_end = (api._event_handle(ev, None) for ev in events)
+            api.wl_eval_seeded(field, cfg.seed, sh.n_loops, cfg.n_ppl, Td, rd, pd, n_groups=sh.n_groups, compute=compute,
+                               storage=tdt, loop_begin=sh.loop_begin, W_mean=W_mean, group_sums=gs_local,
+                               workspace=workspace, options=opt)
+        else:
+            api.wl_eval(field, loops, Td, rd, pd, n_groups=sh.n_groups, compute=compute, W_mean=W_mean,
+                        group_sums=gs_local, workspace=workspace, wilson_events=events, options=options())
         gs = shard.all_gather_group_sums(gs_local, world) if world > 1 else gs_local
         return api.wl_jackknife_finalize(gs, n_loops_total)
 
@@ -265,7 +289,8 @@ def run_ours(args, cfg):
 
     # ---- e2e: the C-ABI call on HOST buffers (wl_eval_host), copies inside the timed region ----
     e2e = None
-    if not args.no_e2e:
+    plain = options() is None
+    if not args.no_e2e and plain:
         host_loops = torch.empty(loops.shape, dtype=loops.dtype, pin_memory=True)
         host_loops.copy_(loops)
         torch.cuda.synchronize()
@@ -301,27 +326,51 @@ def run_ours(args, cfg):
     # ---- roofline of the dominant kernel (k_wilson), DESIGN.md section 5 ----
     sm_max_mhz = clocks.get("sm_max_mhz") or 1965
     k_ms = sum(wilson_ms) / len(wilson_ms)
+    Q = args.quadrature
+    pipe_frac = None          # the binding pipe's utilisation by the instructions the kernel really issues
     if compute == "f32":
-        ops = (ALG_PLAIN_OPS + ALG_SFU_OPS) if cfg.profile == 1 else ALG_OPS_UNIFORM
+        if cfg.profile == 1:
+            ops = ALG_PLAIN_OPS + ALG_SFU_OPS + (Q - 1) * (ALG_NODE_PLAIN_OPS + ALG_NODE_SFU_OPS)
+            ops_how = ("%d algorithmic FP32 lane-ops per point-eval (29 plain + 7 special-function, SURVEY.md 8(d)%s)"
+                       % (ops, "" if Q == 1 else "; + 21 + 4 per extra Gauss-Legendre node"))
+            pipe_frac = {"pipe": "xu", "ops_per_point_eval": KERNEL_SFU_OPS + 2 * (Q - 1),
+                         "peak_lanes_per_clk_sm": SFU_LANES_PER_CLK_SM}
+        else:
+            ops = ALG_OPS_UNIFORM
+            ops_how = "%d algorithmic FP32 lane-ops per point-eval (uniform field: the bare cross product)" % ops
         peak = SM_COUNT * ISSUE_LANES_PER_CLK_SM * sm_max_mhz * 1e6
-        peak_how = ("derived: 148 SMs x 4 sub-partitions x 32 lanes x %d MHz (FP32 non-tensor issue roofline; "
-                    "FFMA micro-benchmark measured 123/128 of it, profiles/r01_pipe_rates.md)" % sm_max_mhz)
-        ops_how = "%d algorithmic FP32 lane-ops per point-eval (29 plain + 7 special-function, SURVEY.md 8(d))" % ops
+        peak_how = ("derived: 148 SMs x 4 sub-partitions x 32 lanes x %d MHz (FP32 non-tensor issue roofline, the "
+                    "north_star denominator; FFMA micro-benchmark measured 123-127 of 128 lanes/clk/SM, "
+                    "profiles/r01_pipe_rates.md). Packed FFMA2 does not raise the FMA-pipe rate; XU and ALU-pipe work "
+                    "can overlap it, so the binding pipe's own utilisation is given in pipe_frac" % sm_max_mhz)
     else:
-        ops = ALG_F64_OPS_SECH2 if cfg.profile == 1 else ALG_OPS_UNIFORM
+        if cfg.profile == 1:
+            ops = ALG_F64_OPS_SECH2
+            ops_how = ("%d FP64 lane-ops per point-eval counted from the mathematics (29 plain + 72 for the seven "
+                       "elementary functions as shortest double-precision sequences, DESIGN.md section 5)" % ops)
+            if Q == 1:
+                pipe_frac = {"pipe": "fp64", "ops_per_point_eval": KERNEL_F64_OPS_SECH2,
+                             "peak_lanes_per_clk_sm": FP64_LANES_PER_CLK_SM}
+        else:
+            ops = ALG_OPS_UNIFORM
+            ops_how = "%d algorithmic FP64 lane-ops per point-eval (uniform field)" % ops
         peak = SM_COUNT * FP64_LANES_PER_CLK_SM * sm_max_mhz * 1e6
-        peak_how = "derived: 148 SMs x 64 FP64 lanes x %d MHz (DFMA micro-benchmark measured 63.8/64)" % sm_max_mhz
-        ops_how = "%d FP64 lane-ops per point-eval (DESIGN.md section 5)" % ops
+        peak_how = "derived: 148 SMs x 64 FP64 lanes x %d MHz (DFMA micro-benchmark measured 62-63.8 of 64)" % sm_max_mhz
     achieved = ops * evals_per_gpu / (k_ms * 1e-3)
+    if pipe_frac is not None:
+        pipe_frac["frac"] = (pipe_frac["ops_per_point_eval"] * evals_per_gpu / (k_ms * 1e-3)) / (
+            SM_COUNT * pipe_frac["peak_lanes_per_clk_sm"] * sm_max_mhz * 1e6)
+        pipe_frac["note"] = "instructions the kernel issues on its binding pipe (not an algorithmic count)"
+    traffic, traffic_note = ncu_traffic(cfg.name, compute, args)
     roofline = {
         "bound": "alu", "kernel": "k_wilson", "achieved": achieved / 1e12, "peak": peak / 1e12,
-        "unit": "Tlane-op/s", "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES.get((cfg.name, compute)),
+        "unit": "Tlane-op/s", "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_note,
         "kernel_ms": k_ms, "kernel_share_of_step": k_ms / ms_per_step,
-        "algorithmic_ops": ops_how, "peak_source": peak_how,
-        # the special-function ops the kernel really issues (5 per point-eval) against the measured XU rate
-        "xu_pipe_frac": (KERNEL_SFU_OPS * evals_per_gpu / (k_ms * 1e-3)) / (SM_COUNT * SFU_LANES_PER_CLK_SM * sm_max_mhz * 1e6)
-        if (compute == "f32" and cfg.profile == 1 and phi is None) else None,
-        "hbm_GBps_algorithmic": loops.numel() * loops.element_size() / (k_ms * 1e-3) / 1e9,
+        "algorithmic_ops": ops_how, "peak_source": peak_how, "pipe_frac": pipe_frac,
+        "xu_pipe_frac": pipe_frac["frac"] if (pipe_frac and pipe_frac["pipe"] == "xu") else None,
+        "fp64_pipe_frac": pipe_frac["frac"] if (pipe_frac and pipe_frac["pipe"] == "fp64") else None,
+        "algorithmic_bytes": (0 if seeded else loop_bytes) + ws_bytes,
+        "hbm_GBps_algorithmic": (0 if seeded else loop_bytes) / (k_ms * 1e-3) / 1e9,
     }
 
     # ---- cpu_baseline: the oracle as it stands, bounded sample, this box's host cores ----
@@ -329,16 +378,19 @@ def run_ours(args, cfg):
     if not args.no_cpu_baseline:
         cores = affinity_cores()
         n = oracle_sample_loops(cfg, cores, 256)
-        sample_loops = loops[:n].cpu().numpy()
+        sample_loops = (loops[:n] if loops is not None else
+                        api.wl_loops_generate(n, cfg.n_ppl, cfg.seed, tdt, loop_begin=sh.loop_begin)).cpu().numpy()
         rate, dt, threads = time_oracle(cfg, sample_loops, T, rho, phi)
         cpu_baseline = {"value": rate, "unit": UNIT, "cores": threads, "kind": "oracle",
                         "sample": "first %d whole loops x full %dx%d grid (%.1f s)" % (n, cfg.n_T, cfg.n_rho, dt)}
 
-    launches_per_step = api.wl_eval_launch_count(sh.n_loops, cfg.n_ppl, cfg.n_T, cfg.n_rho, sh.n_groups, compute) + 1
+    launches_per_step = (api.wl_eval_launch_count(sh.n_loops, cfg.n_ppl, cfg.n_T, cfg.n_rho, sh.n_groups, compute) + 1
+                         + (1 if args.shuffle else 0))      # + k_jackknife_finalize (+ k_group_permutation)
     line = base_line(args, cfg, world)
     line.update({
         "value": value, "ms_per_step": ms_per_step, "dtype": compute,
-        "config": workload_config(cfg, world, compute),
+        "config": dict(workload_config(cfg, world, compute), loops=args.loops, quadrature_order=args.quadrature,
+                       shuffled_groups=bool(args.shuffle), staging=args.staging),
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
         "roofline": roofline, "cpu_baseline": cpu_baseline,
         "checksum_sum_W_mean": result_checksum,
@@ -350,14 +402,37 @@ def run_ours(args, cfg):
     return 0
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_wilson launch from the `ncu --set full` capture
-# summarised under profiles/ (per launch, like `achieved`); None until measured for that workload.
-NCU_TRAFFIC_BYTES = {
-    # profiles/r01_wilson_f32_ncu.md: 276.9 MB read (the 268.4 MB ensemble once) + 56.5 MB written (partials)
-    ("cfg3_paper_scale", "f32"): 276931072 + 56459264,
-    # profiles/r01_wilson_f64_ncu.md: 4.2 MB read, partials still in L2
-    ("cfg1_small_sech2", "f64"): 4217088,
-}
+def source_sha16():
+    """sha256 (first 16 hex digits) of the kernel sources: ties an ncu capture to the code that was profiled."""
+    import hashlib
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_1407_7486_b200", "csrc")
+    files = sorted(f for f in os.listdir(csrc) if f.endswith((".cu", ".cuh"))) if os.path.isdir(csrc) else []
+    for f in files:
+        with open(os.path.join(csrc, f), "rb") as fh:
+            h.update(f.encode() + b"\0" + fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(workload, compute, args):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one k_wilson launch, from profiles/ncu_traffic.json
+    (written by `python -m paper_1407_7486_b200.ncu_summary` from an `ncu --set full` capture).  null unless the
+    capture was taken on exactly these kernel sources and this (workload, compute, options)."""
+    path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
+    try:
+        with open(path) as fh:
+            tab = json.load(fh)
+    except (OSError, ValueError):
+        return None, "no profiles/ncu_traffic.json"
+    key = "%s/%s" % (workload, compute)
+    if args.loops != "stored" or args.quadrature != 1 or args.shuffle or args.staging != "default":
+        key += "/loops=%s,Q=%d,shuffle=%d,staging=%s" % (args.loops, args.quadrature, int(args.shuffle), args.staging)
+    e = tab.get("entries", {}).get(key)
+    if e is None:
+        return None, "no ncu capture of %s" % key
+    if e.get("source_sha16") != source_sha16():
+        return None, "ncu capture of %s is from other kernel sources (%s)" % (key, e.get("source_sha16"))
+    return int(e["dram_bytes_read"]) + int(e["dram_bytes_write"]), "profiles/ncu_traffic.json: %s (%s)" % (key, e.get("report"))
 
 
 def main():
@@ -368,6 +443,13 @@ def main():
     ap.add_argument("--impl", choices=("ours", "reference"), default="ours")
     ap.add_argument("--workload", type=int, default=3, help="BASELINE.json config number (1-5); 3 = paper scale")
     ap.add_argument("--compute", choices=("f32", "f64"), default=None)
+    ap.add_argument("--loops", choices=("stored", "seeded"), default="stored",
+                    help="seeded: no ensemble buffer, loops regenerated inside k_wilson (wl_eval_seeded)")
+    ap.add_argument("--quadrature", type=int, choices=(1, 2, 3), default=1, help="Gauss-Legendre points of eq. (24)")
+    ap.add_argument("--shuffle", action="store_true", help="shuffled group assignment per proper time")
+    ap.add_argument("--staging", choices=("default", "bulk"), default="default")
+    ap.add_argument("--n-loops", type=int, default=None, help="override the workload's loops per GPU (a multiple of its groups)")
+    ap.add_argument("--loop-dtype", choices=("f32", "f64"), default=None, help="override the loop storage precision")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -375,6 +457,12 @@ def main():
         raise SystemExit("--steps >= 1, --warmup >= 0")
     from paper_1407_7486_b200 import inputs
     cfg = inputs.config(args.workload)
+    if args.n_loops is not None or args.loop_dtype is not None:
+        import dataclasses
+        cfg = dataclasses.replace(cfg, name=cfg.name + "_variant", n_loops=args.n_loops or cfg.n_loops,
+                                  loop_dtype=args.loop_dtype or cfg.loop_dtype)
+        if cfg.n_loops % cfg.n_groups != 0:
+            raise SystemExit("--n-loops must be a multiple of the workload's %d groups" % cfg.n_groups)
     if args.impl == "reference":
         return run_reference(args, cfg)
     return run_ours(args, cfg)

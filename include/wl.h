@@ -112,7 +112,7 @@ size_t wl_eval_workspace_bytes(int64_t n_loops, int n_ppl, int n_T, int n_rho, i
  * non-finite value gives NaN rows, not an error.  wl_grid_validate checks a host copy.
  * compute = WL_F64: all arithmetic FP64.  compute = WL_F32: per-term arithmetic
  * FP32 with fast intrinsics, the sums round a loop accumulated in FP64 from
- * FP32 partials of 32 terms, cos/cosh and all sums over loops FP64.
+ * FP32 partials of at most 128 terms, cos/cosh and all sums over loops FP64.
  * Errors: null pointers, sizes < 1, n_groups < 1, n_loops % n_groups != 0
  * (equal groups are required), n_T * n_rho > 2^24, more than 2^31 - 1 CTAs
  * -> WL_ERR_INVALID_ARG; workspace too small -> WL_ERR_WORKSPACE. */

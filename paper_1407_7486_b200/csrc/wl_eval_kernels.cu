@@ -90,9 +90,10 @@ EvalPlan make_eval_plan(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_gr
     // a 148-SM part over many waves.  A function of the sizes only: the summation order, and
     // with it every bit of the result, is the same on any device.
     p.loops_per_unit = 1;
+    const int64_t min_ctas = 16384;         // ~28 waves of 592 resident CTAs: the last, partial wave costs < 1 %
     if (!per_loop) {
         for (int d = 8; d > 1; --d)
-            if (per_group % d == 0 && (n_loops / d) * p.n_tiles >= 4096) { p.loops_per_unit = d; break; }
+            if (per_group % d == 0 && (n_loops / d) * p.n_tiles >= min_ctas) { p.loops_per_unit = d; break; }
     }
     p.n_units = n_loops / p.loops_per_unit;
     p.units_per_group = per_group / p.loops_per_unit;

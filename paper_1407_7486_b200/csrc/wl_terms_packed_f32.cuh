@@ -48,7 +48,7 @@ template <int P_, int THREADS_, bool HAS_PHI, int Q_, int MINB_>
 struct PackedF32Base {
     static_assert(P_ % 2 == 0, "grid points are processed as register pairs");
     static_assert(Q_ >= 1 && Q_ <= 3, "1-, 2- or 3-point Gauss-Legendre rule");
-    static constexpr int kP = P_, kThreads = THREADS_, kMinBlocks = MINB_, kChunk = 1024, kSumBlock = 32, kUnroll = 2;
+    static constexpr int kP = P_, kThreads = THREADS_, kMinBlocks = MINB_, kChunk = 1024, kSumBlock = 128, kUnroll = 2;
     static constexpr bool kHasPhi = HAS_PHI;
     static constexpr int kQ = Q_;
     static constexpr int NP = P_ / 2;                         // register pairs per thread
@@ -116,31 +116,47 @@ struct PackedF32Base {
         if (HAS_PHI) w = fma2(g.ay[q], pk1(v[at + 1]), w);
         return fma2(g.Tt[q], pk1(v[at + C - 1]), w);
     }
-    // (scaled) x_i x x_{i+1} for pair q: ax dy_y/2 - [ay dy_x/2] + Tt (y_i x y_{i+1}); eq. (24)
-    __device__ __forceinline__ static u64 cross(const Grid& g, int q, const float (&v)[NFP])
-    {
-        u64 c = mul2(g.Tt[q], pk1(v[iCR + C - 1]));
-        if (HAS_PHI) c = fma2(g.ay[q], pk1(-v[iCR + 1]), c);
-        return fma2(g.ax[q], pk1(v[iCR]), c);
-    }
-
-    // FP32 partial sums of one block of kSumBlock terms (reading A8)
+    // FP32 partial sums of one block of kSumBlock = 128 terms (reading A8).  The phase sum is kept as C
+    // sums  sum_i g_i dy_y/2, [sum_i g_i dy_x/2], sum_i g_i (y_i x y_{i+1})  and the grid-point factors (ax, ay, Tt)
+    // of the cross product, eq. (24), are applied once per block in FP64: two two-source FFMA2 per pair instead of
+    // FMUL2 + FFMA2 + a three-source FFMA2 (3 clk on the FMA pipe, profiles/r01_pipe_rates.md).
     struct Acc {
-        u64 ph[NP], sp[NP];
+        u64 ph[NP][C], sp[NP];
         __device__ __forceinline__ void zero()
         {
 #pragma unroll
-            for (int q = 0; q < NP; ++q) { ph[q] = 0ull; sp[q] = 0ull; }       // (+0.0f, +0.0f)
+            for (int q = 0; q < NP; ++q) {
+                sp[q] = 0ull;                                                   // (+0.0f, +0.0f)
+#pragma unroll
+                for (int k = 0; k < C; ++k) ph[q][k] = 0ull;
+            }
         }
-        __device__ __forceinline__ void flush(const Grid&, double (&dph)[P_], double (&dsp)[P_]) const
+        __device__ __forceinline__ void add_phase(int q, u64 gt, const float (&v)[NFP])
+        {
+#pragma unroll
+            for (int k = 0; k < C; ++k) ph[q][k] = fma2(gt, pk1(v[iCR + k]), ph[q][k]);
+        }
+        __device__ __forceinline__ void flush(const Grid& g, double (&dph)[P_], double (&dsp)[P_]) const
         {
 #pragma unroll
             for (int q = 0; q < NP; ++q) {
-                float p0, p1, s0, s1;
-                upk(ph[q], p0, p1);
+                float s0, s1, a0, a1, t0, t1, y0, y1, c0, c1;
                 upk(sp[q], s0, s1);
-                dph[2 * q] += double(p0); dph[2 * q + 1] += double(p1);
                 dsp[2 * q] += double(s0); dsp[2 * q + 1] += double(s1);
+                upk(g.ax[q], a0, a1);
+                upk(g.Tt[q], t0, t1);
+                upk(ph[q][0], y0, y1);
+                upk(ph[q][C - 1], c0, c1);
+                double d0 = double(a0) * double(y0) + double(t0) * double(c0);
+                double d1 = double(a1) * double(y1) + double(t1) * double(c1);
+                if (HAS_PHI) {
+                    float b0, b1, x0, x1;
+                    upk(g.ay[q], b0, b1);
+                    upk(ph[q][HAS_PHI ? 1 : 0], x0, x1);
+                    d0 -= double(b0) * double(x0);
+                    d1 -= double(b1) * double(x1);
+                }
+                dph[2 * q] += d0; dph[2 * q + 1] += d1;
             }
         }
     };
@@ -171,7 +187,7 @@ struct PackedF32Base {
 // sech^2 profile.  Scaling: with k = 2 log2(e)/lambda all squared radii are carried as w' = k^2 w, so that
 // u' = sqrt(w') = 2 log2(e) rho/lambda and E = exp(-2 rho/lambda) = 2^(-u') need no multiply, and
 //   h(u)    = ln2 [ (1 - log2(1+E)) - u' E/(1+E) ] / u^2  = 4 log2(e) * br / w'
-//   x_i x x_{i+1} carried times k^2
+//   x_i x x_{i+1} carried times k^2 (through ax, ay, Tt at the end of every block)
 // hence phase = eB0 * lambda^2 ln2 * sum_i [sum_q w_q br/w'](i) * [k^2 x_i x x_{i+1}](i): the constants leave the loop.
 // Near the axis (w = u^2 < 1/8) the bracket cancels and a degree-3 polynomial in w' replaces br/w'
 // (coefficients: gen_h_poly.py hs 0.125 3, relative error 8e-8).
@@ -291,7 +307,7 @@ struct Sech2PackedF32 : PackedF32Base<P_, THREADS_, HAS_PHI, Q_, MINB_> {
                 gt = add2(gt, g_node(wm[2], rm[2], um[2], Em[2], imn[2]));
                 gt = fma2(g_node(wm[1], rm[1], um[1], Em[1], imn[1]), pk1(1.6f), gt);
             }
-            acc.ph[q] = fma2(gt, B::cross(g, q, v), acc.ph[q]);
+            acc.add_phase(q, gt, v);
         }
     }
 };
@@ -354,7 +370,7 @@ struct FluxTubePackedF32 : PackedF32Base<P_, THREADS_, HAS_PHI, Q_, MINB_> {
                 gt = mul2(rDp, fma2(mul2(am[0], am[2]), pk1(1.6f), mul2(am[1], add2(am[0], am[2]))));
             }
             acc.sp[q] = fma2(ip, ip, acc.sp[q]);                              // 1/a_p^2        -> b
-            acc.ph[q] = fma2(gt, B::cross(g, q, v), acc.ph[q]);
+            acc.add_phase(q, gt, v);
         }
     }
 };

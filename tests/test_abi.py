@@ -82,8 +82,8 @@ def test_workspace_plan_is_a_function_of_sizes_only(lib):
     f = lib.wl_eval_workspace_bytes
     f.restype = C.c_size_t
     f.argtypes = [C.c_int64, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int]
-    # config 3: 16384 loops, 64x64 grid, G = 64: units of 8 loops -> 2048 x 4096 doubles
-    assert f(16384, 2048, 64, 64, 64, 0) == 2048 * 4096 * 8
+    # config 3: 16384 loops, 64x64 grid, G = 64: units of 4 loops -> 4096 x 4096 doubles
+    assert f(16384, 2048, 64, 64, 64, 0) == 4096 * 4096 * 8
     # a partial is never coarser than a group and never finer than a loop
     for (nl, g, nt, nr) in ((1024, 16, 16, 16), (4096, 32, 32, 8), (65536, 256, 64, 64), (12, 4, 3, 5), (7, 7, 1, 1)):
         b = f(nl, 64, nt, nr, g, 1)
