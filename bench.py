@@ -209,7 +209,10 @@ def run_ours(args, cfg):
                              % args.gpus)
         raise SystemExit("WORLD_SIZE %d != --gpus %d" % (world, args.gpus))
     torch.cuda.set_device(local_rank)
-    if world > 1:
+    # under torch.distributed.run the process group is set up even for one rank, so that the collective path
+    # (all-gather of the group sums, barriers, MAX over ranks) is the one that runs
+    use_dist = world > 1 or "TORCHELASTIC_RUN_ID" in os.environ
+    if use_dist:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     compute = args.compute or ("f32" if "f32" in cfg.compute else "f64")
@@ -224,11 +227,12 @@ def run_ours(args, cfg):
     loop_bytes = sh.n_loops * cfg.n_ppl * 2 * (4 if cfg.loop_dtype == "f32" else 8)
 
     def options():
-        if args.quadrature == 1 and not args.shuffle and args.staging == "default" and not seeded:
+        if args.quadrature == 1 and not args.shuffle and args.staging == "default" and not seeded and world == 1:
             return None
         return api.wl_eval_options(quadrature_order=args.quadrature, shuffle_seed=(cfg.seed + 1000 if args.shuffle else None),
                                    staging=(1 if args.staging == "bulk" else 0),
-                                   seed=(cfg.seed if seeded else None), loop_begin=sh.loop_begin)
+                                   seed=(cfg.seed if seeded else None), loop_begin=sh.loop_begin,
+                                   ensemble_loops=(sh.n_loops * world if world > 1 else 0))
     ws_bytes = api.wl_eval_opt_workspace_bytes(sh.n_loops, cfg.n_ppl, cfg.n_T, cfg.n_rho, sh.n_groups, compute, options())
     workspace = torch.empty(max(ws_bytes, 8), dtype=torch.uint8, device="cuda")
     W_mean = torch.empty((cfg.n_T, cfg.n_rho), dtype=torch.float64, device="cuda")
@@ -247,12 +251,12 @@ def run_ours(args, cfg):
         else:
             api.wl_eval(field, loops, Td, rd, pd, n_groups=sh.n_groups, compute=compute, W_mean=W_mean,
                         group_sums=gs_local, workspace=workspace, wilson_events=events, options=options())
-        gs = shard.all_gather_group_sums(gs_local, world) if world > 1 else gs_local
+        gs = shard.all_gather_group_sums(gs_local, world) if use_dist else gs_local
         return api.wl_jackknife_finalize(gs, n_loops_total)
 
     def fence():
         torch.cuda.synchronize()
-        if world > 1:
+        if use_dist:
             dist.barrier()
             torch.cuda.synchronize()
 
@@ -276,7 +280,7 @@ def run_ours(args, cfg):
     clocks = sampler.stop()
     ms_total = e0.elapsed_time(e1)
     wilson_ms = [a.elapsed_time(b) for a, b in k_events]
-    if world > 1:
+    if use_dist:
         t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms_total = float(t.item())
@@ -289,7 +293,7 @@ def run_ours(args, cfg):
 
     # ---- e2e: the C-ABI call on HOST buffers (wl_eval_host), copies inside the timed region ----
     e2e = None
-    plain = options() is None
+    plain = args.quadrature == 1 and not args.shuffle and args.staging == "default" and not seeded
     if not args.no_e2e and plain:
         host_loops = torch.empty(loops.shape, dtype=loops.dtype, pin_memory=True)
         host_loops.copy_(loops)
@@ -303,7 +307,7 @@ def run_ours(args, cfg):
         for _ in range(args.steps):
             hm, he, hg = api.wl_eval_host(field, hl, T, rho, phi, n_groups=G_e2e, compute=compute)
         dt = time.perf_counter() - t0
-        if world > 1:
+        if use_dist:
             t = torch.tensor([dt], dtype=torch.float64, device="cuda")
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             dt = float(t.item())
@@ -318,7 +322,7 @@ def run_ours(args, cfg):
         del host_loops
 
     if rank != 0:
-        if world > 1:
+        if use_dist:
             dist.barrier()
             dist.destroy_process_group()
         return 0
@@ -396,7 +400,7 @@ def run_ours(args, cfg):
         "checksum_sum_W_mean": result_checksum,
     })
     print(json.dumps(line), flush=True)
-    if world > 1:
+    if use_dist:
         dist.barrier()
         dist.destroy_process_group()
     return 0

@@ -155,6 +155,11 @@ wl_status wl_grid_validate(const double* h_T, int n_T, const double* h_rho_cm, i
  *   two-slot shared-memory ring with mbarrier completion, one chunk ahead of the evaluation
  *   (compiled for the main kernels only, silently 0 elsewhere; same bits either way).
  *
+ * ensemble_loops: 0, or the number of loops of the whole ensemble when this call evaluates one shard of it
+ *   (whole jackknife groups).  The work is then cut into the same units of loops as
+ *   in one call over the whole ensemble, so every group sum has the same bits however many shards there are.
+ *   Must be a multiple of n_loops' group size and >= n_loops, else WL_ERR_INVALID_ARG.
+ *
  * event_wilson_begin / event_wilson_end: optional cudaEvent_t (as void*) recorded on the stream
  *   immediately before and after the k_wilson launch. */
 typedef struct wl_eval_options {
@@ -166,6 +171,7 @@ typedef struct wl_eval_options {
     int shuffle_groups;
     int staging;
     uint64_t shuffle_seed;
+    int64_t ensemble_loops;
     void* event_wilson_begin;
     void* event_wilson_end;
 } wl_eval_options;

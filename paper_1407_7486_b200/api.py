@@ -52,7 +52,7 @@ class _Options(C.Structure):
     """struct wl_eval_options of include/wl.h."""
     _fields_ = [("struct_size", C.c_size_t), ("quadrature_order", C.c_int), ("seeded", C.c_int),
                 ("seed", C.c_uint64), ("loop_begin", C.c_int64), ("shuffle_groups", C.c_int), ("staging", C.c_int),
-                ("shuffle_seed", C.c_uint64), ("event_wilson_begin", C.c_void_p), ("event_wilson_end", C.c_void_p)]
+                ("shuffle_seed", C.c_uint64), ("ensemble_loops", C.c_int64), ("event_wilson_begin", C.c_void_p), ("event_wilson_end", C.c_void_p)]
 
 
 _op = C.POINTER(_Options)
@@ -215,8 +215,10 @@ def _event_handle(ev, stream):
     return C.c_void_p(ev.cuda_event)
 
 
-def wl_eval_options(quadrature_order=1, seed=None, loop_begin=0, shuffle_seed=None, staging=0) -> _Options:
-    """struct wl_eval_options: seed != None sets `seeded`, shuffle_seed != None sets `shuffle_groups`."""
+def wl_eval_options(quadrature_order=1, seed=None, loop_begin=0, shuffle_seed=None, staging=0,
+                    ensemble_loops=0) -> _Options:
+    """struct wl_eval_options: seed != None sets `seeded`, shuffle_seed != None sets `shuffle_groups`;
+    ensemble_loops = size of the whole ensemble when the call evaluates one shard of it."""
     o = _Options()
     _lib.wl_eval_options_default(C.byref(o))
     o.quadrature_order = int(quadrature_order)
@@ -225,6 +227,7 @@ def wl_eval_options(quadrature_order=1, seed=None, loop_begin=0, shuffle_seed=No
     if shuffle_seed is not None:
         o.shuffle_groups, o.shuffle_seed = 1, int(shuffle_seed)
     o.staging = int(staging)
+    o.ensemble_loops = int(ensemble_loops)
     return o
 
 

@@ -31,6 +31,7 @@ struct Opt {
     int quad = 1, seeded = 0, shuffle = 0, bulk = 0;
     uint64_t seed = 0, shuffle_seed = 0;
     int64_t loop_begin = 0;
+    int64_t ensemble_loops = 0;      // 0: this call is the whole ensemble
     void* ev0 = nullptr;
     void* ev1 = nullptr;
 };
@@ -50,6 +51,8 @@ bool read_options(const wl_eval_options* o, int n_ppl, int64_t n_loops, Opt* out
     if (out->shuffle && n_loops > 0x7fffffffLL) return false;
     if (o->staging != 0 && o->staging != 1) return false;
     out->bulk = o->staging;
+    if (o->ensemble_loops < 0 || (o->ensemble_loops > 0 && o->ensemble_loops < n_loops)) return false;
+    out->ensemble_loops = o->ensemble_loops;
     out->ev0 = o->event_wilson_begin;
     out->ev1 = o->event_wilson_end;
     return true;
@@ -153,7 +156,8 @@ size_t wl_eval_opt_workspace_bytes(int64_t n_loops, int n_ppl, int n_T, int n_rh
     if (!sizes_ok(n_loops, n_ppl, n_T, n_rho, n_groups) || !dtype_ok(compute)) return 0;
     Opt o;
     if (!read_options(opt, n_ppl, n_loops, &o)) return 0;
-    const EvalPlan p = make_eval_plan(n_loops, n_ppl, n_T, n_rho, n_groups, compute, o.shuffle != 0);
+    if (o.ensemble_loops % (n_loops / n_groups) != 0) return 0;
+    const EvalPlan p = make_eval_plan(n_loops, n_ppl, n_T, n_rho, n_groups, compute, o.shuffle != 0, o.ensemble_loops);
     const size_t partial = (size_t)p.n_units * (size_t)p.n_grid * sizeof(double);
     if (!o.shuffle) return partial;
     return align256(partial) + align256((size_t)n_T * (size_t)n_loops * sizeof(int32_t));   // W per loop, membership table
@@ -214,9 +218,11 @@ wl_status wl_eval_opt(const wl_field* field, const void* d_loops, wl_dtype loop_
     Opt o;
     if (!read_options(opt, n_ppl, n_loops, &o)) return WL_ERR_INVALID_ARG;
     if (!o.seeded && !d_loops) return WL_ERR_INVALID_ARG;
+    if (o.shuffle && o.ensemble_loops > 0) return WL_ERR_UNSUPPORTED;     // a shard cannot shuffle across shards
     const size_t need = wl_eval_opt_workspace_bytes(n_loops, n_ppl, n_T, n_rho, n_groups, compute, opt);
+    if (need == 0) return WL_ERR_INVALID_ARG;
     if (!d_workspace || workspace_bytes < need) return WL_ERR_WORKSPACE;
-    const EvalPlan plan = make_eval_plan(n_loops, n_ppl, n_T, n_rho, n_groups, compute, o.shuffle != 0);
+    const EvalPlan plan = make_eval_plan(n_loops, n_ppl, n_T, n_rho, n_groups, compute, o.shuffle != 0, o.ensemble_loops);
 
     EvalArgs a = make_args(field, d_loops, loop_dtype, n_loops, n_ppl, d_T, n_T, d_rho_cm, d_phi_cm, n_rho, o);
     a.partial = reinterpret_cast<double*>(d_workspace);

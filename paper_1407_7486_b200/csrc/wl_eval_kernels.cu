@@ -75,7 +75,7 @@ __global__ void k_group_reduce_shuffled(const double* __restrict__ W_loop, const
 // ------------------------------------------------------------------ host side: plan + dispatch
 
 EvalPlan make_eval_plan(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups, wl_dtype compute,
-                        bool per_loop)
+                        bool per_loop, int64_t ensemble_loops)
 {
     (void)n_ppl;
     EvalPlan p;
@@ -86,6 +86,7 @@ EvalPlan make_eval_plan(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_gr
     while (p.P < p_max && p.n_grid >= kThreads * p.P * 2) p.P *= 2;
     p.n_tiles = (p.n_grid + kThreads * p.P - 1) / (kThreads * p.P);
     const int64_t per_group = n_loops / n_groups;
+    const int64_t all_loops = ensemble_loops > 0 ? ensemble_loops : n_loops;
     // Largest divisor of the group size, at most 8, that still leaves enough CTAs to balance
     // a 148-SM part over many waves.  A function of the sizes only: the summation order, and
     // with it every bit of the result, is the same on any device.
@@ -93,7 +94,7 @@ EvalPlan make_eval_plan(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_gr
     const int64_t min_ctas = 16384;         // ~28 waves of 592 resident CTAs: the last, partial wave costs < 1 %
     if (!per_loop) {
         for (int d = 8; d > 1; --d)
-            if (per_group % d == 0 && (n_loops / d) * p.n_tiles >= min_ctas) { p.loops_per_unit = d; break; }
+            if (per_group % d == 0 && (all_loops / d) * p.n_tiles >= min_ctas) { p.loops_per_unit = d; break; }
     }
     p.n_units = n_loops / p.loops_per_unit;
     p.units_per_group = per_group / p.loops_per_unit;

@@ -29,8 +29,10 @@ struct EvalPlan {
     int64_t units_per_group; // (n_loops / n_groups) / loops_per_unit
 };
 
+// ensemble_loops > 0: n_loops is a shard (whole groups) of an ensemble of that many loops; the units are those
+// of a call over the whole ensemble.
 EvalPlan make_eval_plan(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups, wl_dtype compute,
-                        bool per_loop);
+                        bool per_loop, int64_t ensemble_loops = 0);
 
 struct EvalArgs {
     const void* loops;          // [n_loops][n_ppl][2]; unused when seeded

@@ -48,8 +48,14 @@ def all_gather_group_sums(local_group_sums: torch.Tensor, world_size: int, group
     local = local_group_sums.contiguous()
     g_local = local.shape[0]
     out = torch.empty((world_size * g_local,) + tuple(local.shape[1:]), dtype=local.dtype, device=local.device)
-    if world_size == 1:
+    if world_size == 1 and not (dist.is_available() and dist.is_initialized()):
         out.copy_(local)
+        return out
+    if local.is_cuda and dist.get_backend(group) == "gloo":
+        # gloo has no all_gather for CUDA tensors: stage through the host (<= 2 MB per rank); same values, same order
+        host = torch.empty(out.shape, dtype=out.dtype)
+        dist.all_gather([host[r * g_local:(r + 1) * g_local] for r in range(world_size)], local.cpu(), group=group)
+        out.copy_(host)
         return out
     parts = [out[r * g_local:(r + 1) * g_local] for r in range(world_size)]
     dist.all_gather(parts, local, group=group)
@@ -57,7 +63,7 @@ def all_gather_group_sums(local_group_sums: torch.Tensor, world_size: int, group
 
 
 def wl_eval_sharded(field, local_loops, T, rho_cm, phi_cm, shard: Shard, compute, stream=None, group=None,
-                    workspace=None):
+                    workspace=None, options=None):
     """wl_eval on this rank's loops, all-gather of the group sums, finalise on every rank.
 
     local_loops: this rank's loops [shard.n_loops][n_ppl][2] (CUDA).  Returns (mean, err, group_sums)
@@ -66,8 +72,11 @@ def wl_eval_sharded(field, local_loops, T, rho_cm, phi_cm, shard: Shard, compute
     from . import api
     if local_loops.shape[0] != shard.n_loops:
         raise ValueError("local_loops has %d loops, the shard owns %d" % (local_loops.shape[0], shard.n_loops))
+    # the units of loops are those of one call over the whole ensemble: same bits for any number of ranks
+    opt = options if options is not None else api.wl_eval_options()
+    opt.ensemble_loops = shard.n_loops * shard.world_size
     _, gs_local = api.wl_eval(field, local_loops, T, rho_cm, phi_cm, n_groups=shard.n_groups, compute=compute,
-                              stream=stream, workspace=workspace)
+                              stream=stream, workspace=workspace, options=opt)
     gs = all_gather_group_sums(gs_local, shard.world_size, group=group)
     mean, err = api.wl_jackknife_finalize(gs, shard.n_loops * shard.world_size, stream=stream)
     return mean, err, gs

@@ -2,7 +2,8 @@
 the whole grid and ensemble), checked on sampled outputs the oracle can compute one by one
 (SURVEY.md section 8(d) coverage table, readings A12):
 
-  config 3: full grid on the GPU; oracle on an 8 x 8 seeded sub-grid x ALL loops      (<W>, S_g)
+  config 3: full grid on the GPU; oracle on a 16 x 16 sub-grid (256 points: both ends of both axes forced in,
+            the rest seeded) x ALL loops                                               (<W>, S_g)
   config 4: FP32 kernel full grid; FP64 kernel on the sub-grid; oracle on the same 8 x 8 sub-grid
   config 5: full grid; oracle on 64 seeded (T, rho) points x 16 seeded WHOLE groups   (S_g)
 """
@@ -28,10 +29,14 @@ def o():
     return wl_oracle
 
 
-def subgrid(c, n_t, n_r, seed):
+def subgrid(c, n_t, n_r, seed, edges=False):
+    """Seeded sub-grid; edges=True forces the first and last index of both axes in (rho_cm = 0 is where the
+    near-axis branch of the sech^2 kernels carries most terms; T_min and T_max are the extremes of the scaling)."""
     rng = np.random.default_rng(seed)
-    ti = np.sort(rng.choice(c.n_T, n_t, replace=False))
-    ri = np.sort(rng.choice(c.n_rho, n_r, replace=False))
+    if not edges:
+        return np.sort(rng.choice(c.n_T, n_t, replace=False)), np.sort(rng.choice(c.n_rho, n_r, replace=False))
+    ti = np.sort(np.concatenate(([0, c.n_T - 1], 1 + rng.choice(c.n_T - 2, n_t - 2, replace=False))))
+    ri = np.sort(np.concatenate(([0, c.n_rho - 1], 1 + rng.choice(c.n_rho - 2, n_r - 2, replace=False))))
     return ti, ri
 
 
@@ -42,9 +47,14 @@ def test_config3_full_fp32_sampled_grid_all_loops(api, o):
     f = api.wl_field_create(c.profile, c.params)
     mean, gs = api.wl_eval(f, loops, dev(T), dev(rho), None, n_groups=c.n_groups, compute="f32")
     mean2, gs2 = api.wl_eval(f, loops, dev(T), dev(rho), None, n_groups=c.n_groups, compute="f32")
+    # seeded evaluation: no ensemble buffer, same bits as generate + eval
+    mean3, gs3 = api.wl_eval_seeded(f, c.seed, c.n_loops, c.n_ppl, dev(T), dev(rho), None, n_groups=c.n_groups,
+                                    compute="f32", storage=torch.float32)
     torch.cuda.synchronize()
     assert torch.equal(gs, gs2) and torch.equal(mean, mean2)          # fixed summation order: same bits
-    ti, ri = subgrid(c, 8, 8, 303)
+    assert torch.equal(gs, gs3) and torch.equal(mean, mean3)
+    ti, ri = subgrid(c, 16, 16, 303, edges=True)          # 256 grid points x all loops (~16 s of oracle)
+    assert ti[0] == 0 and ti[-1] == c.n_T - 1 and ri[0] == 0 and ri[-1] == c.n_rho - 1
     ref = o.evaluate(c.profile, c.params, loops.cpu().numpy(), T[ti], rho[ri], None, n_groups=c.n_groups)
     assert_mean_close(mean.cpu().numpy()[np.ix_(ti, ri)], ref["W_mean"], "f32")
     assert_mean_close(gs.cpu().numpy()[:, ti][:, :, ri], ref["group_sums"], "f32",
@@ -85,7 +95,11 @@ def test_config5_large_sweep_sampled_points_and_whole_groups(api, o):
     loops = api.wl_loops_generate(c.n_loops, c.n_ppl, c.seed, torch.float32)
     f = api.wl_field_create(c.profile, c.params)
     mean, gs = api.wl_eval(f, loops, dev(T), dev(rho), None, n_groups=c.n_groups, compute="f32")
+    mean_s, gs_s = api.wl_eval_seeded(f, c.seed, c.n_loops, c.n_ppl, dev(T), dev(rho), None, n_groups=c.n_groups,
+                                      compute="f32", storage=torch.float32)      # 4.3 GB of coordinates never stored
     torch.cuda.synchronize()
+    assert torch.equal(gs, gs_s) and torch.equal(mean, mean_s)
+    del gs_s, mean_s
     gs = gs.cpu().numpy()
     rng = np.random.default_rng(505)
     groups = np.sort(rng.choice(c.n_groups, 16, replace=False))
