@@ -454,9 +454,13 @@ def main():
     ap.add_argument("--staging", choices=("default", "bulk"), default="default")
     ap.add_argument("--n-loops", type=int, default=None, help="override the workload's loops per GPU (a multiple of its groups)")
     ap.add_argument("--loop-dtype", choices=("f32", "f64"), default=None, help="override the loop storage precision")
+    ap.add_argument("--source-sha", action="store_true", help="print the hash of the kernel sources and exit")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
+    if args.source_sha:
+        print(source_sha16())
+        return 0
     if args.steps < 1 or args.warmup < 0:
         raise SystemExit("--steps >= 1, --warmup >= 0")
     from paper_1407_7486_b200 import inputs

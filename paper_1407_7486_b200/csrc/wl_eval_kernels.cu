@@ -119,15 +119,38 @@ static cudaError_t launch_p(const EvalPlan& plan, const EvalArgs& a, cudaStream_
     }
 }
 
+// Uniform field: UniformTerm.  Grids of at most 256 points run 128 threads x 2 grid points; larger ones 256 threads
+// x plan.P.  The bulk-staging measurement variant exists for the config-2 shape (phi_cm given, small grid).
+template <typename Real, bool HAS_PHI>
+static cudaError_t launch_uniform_phi(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s)
+{
+    if (a.disc) {
+        if (plan.n_grid <= 256) return launch_term<UniformTerm<Real, HAS_PHI, 2, 128>, true, false>(plan, a, s);
+        return plan.P >= 2 ? launch_term<UniformTerm<Real, HAS_PHI, 2, 256>, true, false>(plan, a, s)
+                           : launch_term<UniformTerm<Real, HAS_PHI, 1, 256>, true, false>(plan, a, s);
+    }
+    if (plan.n_grid <= 256) {
+        if (HAS_PHI && bulk_ok(a)) return launch_term<UniformTerm<Real, true, 2, 128>, false, true>(plan, a, s);
+        return launch_term<UniformTerm<Real, HAS_PHI, 2, 128>, false, false>(plan, a, s);
+    }
+    switch (plan.P) {
+        case 1: return launch_term<UniformTerm<Real, HAS_PHI, 1, 256>, false, false>(plan, a, s);
+        case 2: return launch_term<UniformTerm<Real, HAS_PHI, 2, 256>, false, false>(plan, a, s);
+        default: return launch_term<UniformTerm<Real, HAS_PHI, 4, 256>, false, false>(plan, a, s);
+    }
+}
+
+template <typename Real>
+static cudaError_t launch_uniform(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s)
+{
+    return a.phi ? launch_uniform_phi<Real, true>(plan, a, s) : launch_uniform_phi<Real, false>(plan, a, s);
+}
+
 template <typename Real>
 static cudaError_t launch_r(const EvalPlan& plan, const EvalArgs& a, int profile, cudaStream_t s)
 {
     const bool phi = a.phi != nullptr;
-    if (profile == WL_PROFILE_UNIFORM) {
-        // the bulk-staging measurement variant exists for the config-2 shape only (phi_cm given, P = 1)
-        if (phi && plan.P == 1 && bulk_ok(a)) return launch_term<GenericTerm<Real, Uniform, true, 1>, false, true>(plan, a, s);
-        return phi ? launch_p<Real, Uniform, true>(plan, a, s) : launch_p<Real, Uniform, false>(plan, a, s);
-    }
+    if (profile == WL_PROFILE_UNIFORM && a.quad >= 1) return launch_uniform<Real>(plan, a, s);   // g is constant: any Q is the same sum
     if (profile == WL_PROFILE_SECH2)
         return phi ? launch_p<Real, Sech2, true>(plan, a, s) : launch_p<Real, Sech2, false>(plan, a, s);
     if (profile == WL_PROFILE_FLUXTUBE)

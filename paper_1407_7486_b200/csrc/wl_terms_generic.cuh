@@ -133,3 +133,74 @@ struct GenericTerm {
 };
 
 }  // namespace wl
+
+namespace wl {
+
+// UniformTerm<Real, HAS_PHI, P, THREADS>: the constant field B_z = B, A = (B/2)(-y, x) (config 2 of BASELINE.json).
+// g = eB/2 and b = eB are constants, so a point-eval is the bare cross product of eq. (24),
+//     x_i x x_{i+1} = s (c x dy_i) + T (y_i x y_{i+1}),
+// three (two without phi_cm) FMAs that accumulate straight into the phase sum; the spin sum is the number of
+// terms.  One staged Vec4 (dy_y, dy_x, y_i x y_{i+1}, -) per point feeds 3 P FMAs per thread.  The generic
+// kernel spent 11 warp instructions per point-eval on this (issue-bound, profiles/r02_offtarget.md).
+template <typename Real, bool HAS_PHI, int P_, int THREADS_>
+struct UniformTerm {
+    static constexpr int kP = P_, kThreads = THREADS_, kMinBlocks = 1, kUnroll = 4;
+    static constexpr int kSumBlock = sizeof(Real) == 4 ? 128 : 0;      // FP64: straight accumulation
+    static constexpr int kChunk = sizeof(Real) == 4 ? 1024 : 512;
+    static constexpr bool kHasPhi = HAS_PHI;
+    __host__ __device__ static constexpr size_t stage_bytes(int) { return sizeof(Vec4<Real>) * (size_t)kChunk; }
+
+    double eB;
+    __device__ explicit UniformTerm(const EvalArgs& a) : eB(a.p0) {}
+    struct Grid {
+        Real Tt[P_], scx[P_];
+        Real nscy[HAS_PHI ? P_ : 1];
+        __device__ __forceinline__ void load(const UniformTerm&, const double (&T)[P_], const double (&)[P_],
+                                             const double (&cx)[P_], const double (&cy)[P_])
+        {
+#pragma unroll
+            for (int j = 0; j < P_; ++j) {
+                const double s = sqrt(T[j]);
+                Tt[j] = Real(T[j]);
+                scx[j] = Real(s * cx[j]);
+                if (HAS_PHI) nscy[j] = Real(-(s * cy[j]));
+            }
+        }
+    };
+    struct Acc {
+        Real ph[P_];
+        int n;                                                       // terms in this block: the spin sum of a constant field
+        __device__ __forceinline__ void zero()
+        {
+            n = 0;
+#pragma unroll
+            for (int j = 0; j < P_; ++j) ph[j] = Real(0);
+        }
+        __device__ __forceinline__ void flush(const Grid&, double (&dph)[P_], double (&dsp)[P_]) const
+        {
+#pragma unroll
+            for (int j = 0; j < P_; ++j) { dph[j] += double(ph[j]); dsp[j] += double(n); }
+        }
+    };
+    __device__ double g_scale() const { return 0.5 * eB; }
+    __device__ double b_scale() const { return eB; }
+
+    __device__ __forceinline__ static void stage(unsigned char* s, int i, double yx, double yy, double zx, double zy)
+    {
+        Vec4<Real> cr; cr.a = Real(zy - yy); cr.b = Real(zx - yx); cr.c = Real(yx * zy - yy * zx); cr.d = Real(0);
+        reinterpret_cast<Vec4<Real>*>(s)[i] = cr;
+    }
+    __device__ __forceinline__ static void point(const unsigned char* s, int i, const Grid& g, Acc& acc)
+    {
+        const Vec4<Real> cr = reinterpret_cast<const Vec4<Real>*>(s)[i];
+        ++acc.n;
+#pragma unroll
+        for (int j = 0; j < P_; ++j) {
+            Real p = fma(g.scx[j], cr.a, acc.ph[j]);
+            if (HAS_PHI) p = fma(g.nscy[j], cr.b, p);
+            acc.ph[j] = fma(g.Tt[j], cr.c, p);                       // x_i x x_{i+1}, eq. (24)
+        }
+    }
+};
+
+}  // namespace wl
