@@ -26,8 +26,9 @@ cudaError_t launch_shape(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s
         return launch_term<Sech2PackedF32<P, TH, false, 1>, false, false>(plan, a, s);
     }
     if (phi) return cudaErrorInvalidValue;
-    if (a.quad == 2) return launch_term<Sech2PackedF32<P, TH, false, 2>, false, false>(plan, a, s);
-    if (a.quad == 3) return launch_term<Sech2PackedF32<P, TH, false, 3>, false, false>(plan, a, s);
+    if (P == 4) return cudaErrorInvalidValue;            // Q > 1 runs two grid points per thread (launch_wilson_sech2_f32)
+    if (a.quad == 2) return launch_term<Sech2PackedF32<(P == 4 ? 2 : P), TH, false, 2>, false, false>(plan, a, s);
+    if (a.quad == 3) return launch_term<Sech2PackedF32<(P == 4 ? 2 : P), TH, false, 3>, false, false>(plan, a, s);
     return cudaErrorInvalidValue;
 }
 
@@ -39,7 +40,9 @@ cudaError_t launch_shape(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s
 cudaError_t launch_wilson_sech2_f32(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s)
 {
     if (plan.n_grid <= 256) return launch_shape<2, 128>(plan, a, s);
-    if (plan.P == 2) return launch_shape<2, 256>(plan, a, s);
+    // Q > 1 carries Q times the node state: two grid points per thread (no spills; Q = 2: 253.6 against 261.8 ms on
+    // config 3 with four; Q = 3 is FMA-pipe bound either way)
+    if (plan.P == 2 || a.quad > 1) return launch_shape<2, 256>(plan, a, s);
     if (plan.P == 4) return launch_shape<4, 256>(plan, a, s);
     return cudaErrorInvalidValue;
 }
