@@ -127,3 +127,68 @@ def test_proper_time_nodes_host_call(lib):
     assert T[0] == a and all(abs(x[j] - xa * (n - j) / n) < 1e-15 for j in range(n))
     assert lib.wl_proper_time_nodes(a, Tmax, 7, T) == 1 and lib.wl_proper_time_nodes(0.0, Tmax, 8, T) == 1
     assert lib.wl_proper_time_nodes(a, Tmax, 8, None) == 1
+
+
+class _Options(C.Structure):
+    _fields_ = [("struct_size", C.c_size_t), ("quadrature_order", C.c_int), ("seeded", C.c_int),
+                ("seed", C.c_uint64), ("loop_begin", C.c_int64), ("shuffle_groups", C.c_int), ("staging", C.c_int),
+                ("shuffle_seed", C.c_uint64), ("ensemble_loops", C.c_int64), ("event_wilson_begin", C.c_void_p),
+                ("event_wilson_end", C.c_void_p)]
+
+
+def test_options_block_and_its_workspace_sizes(lib):
+    """struct wl_eval_options (NEXT-4 options): defaults, validation and the workspace each option needs -- host only."""
+    o = _Options()
+    lib.wl_eval_options_default.restype = None
+    lib.wl_eval_options_default(C.byref(o))
+    assert o.struct_size == C.sizeof(_Options) and o.quadrature_order == 1
+    assert (o.seeded, o.shuffle_groups, o.staging, o.ensemble_loops) == (0, 0, 0, 0)
+    lib.wl_eval_options_default(None)                                  # NULL is ignored
+    f = lib.wl_eval_opt_workspace_bytes
+    f.restype = C.c_size_t
+    f.argtypes = [C.c_int64, C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(_Options)]
+    base = f(16384, 2048, 64, 64, 64, 0, None)
+    assert base == f(16384, 2048, 64, 64, 64, 0, C.byref(o)) == 4096 * 4096 * 8
+    o.quadrature_order = 3
+    assert f(16384, 2048, 64, 64, 64, 0, C.byref(o)) == base           # the order needs no workspace
+    o.quadrature_order = 4
+    assert f(16384, 2048, 64, 64, 64, 0, C.byref(o)) == 0
+    o.quadrature_order = 1
+    o.shuffle_groups = 1                                               # W per loop + the membership table
+    assert f(16384, 2048, 64, 64, 64, 0, C.byref(o)) == 16384 * 4096 * 8 + 64 * 16384 * 4
+    o.shuffle_groups = 0
+    o.seeded = 1
+    assert f(16384, 2048, 64, 64, 64, 0, C.byref(o)) == base
+    assert f(16384, 2000, 64, 64, 64, 0, C.byref(o)) == 0              # seeded: N must be a power of two
+    assert f(16384, 131072, 4, 4, 64, 0, C.byref(o)) == 0              # ... of at most 65536
+    o.seeded = 0
+    o.ensemble_loops = 8 * 16384                                       # a shard of a 131072-loop ensemble: units of 8 loops
+    assert f(16384, 2048, 64, 64, 64, 0, C.byref(o)) == 2048 * 4096 * 8
+    o.ensemble_loops = 100                                             # smaller than the shard
+    assert f(16384, 2048, 64, 64, 64, 0, C.byref(o)) == 0
+    o.ensemble_loops = 0
+    o.struct_size = 8                                                  # another ABI generation
+    assert f(16384, 2048, 64, 64, 64, 0, C.byref(o)) == 0
+
+
+def test_grid_validate_and_permutation_argument_checks(lib):
+    dp = C.POINTER(C.c_double)
+    lib.wl_grid_validate.restype = C.c_int
+    lib.wl_grid_validate.argtypes = [dp, C.c_int, dp, C.c_int]
+    T = (C.c_double * 3)(0.01, 1.0, 10.0)
+    rho = (C.c_double * 2)(0.0, 4.0)
+    assert lib.wl_grid_validate(T, 3, rho, 2) == 0
+    for bad in (0.0, -1.0, float("nan"), float("inf")):
+        Tb = (C.c_double * 3)(0.01, bad, 10.0)
+        assert lib.wl_grid_validate(Tb, 3, rho, 2) == 1
+    assert lib.wl_grid_validate(T, 3, (C.c_double * 2)(0.0, -1e-12), 2) == 1
+    assert lib.wl_grid_validate(None, 3, rho, 2) == 1 and lib.wl_grid_validate(T, 0, rho, 2) == 1
+    lib.wl_group_permutation.restype = C.c_int
+    lib.wl_group_permutation.argtypes = [C.c_uint64, C.c_int64, C.c_int, C.c_void_p, C.c_void_p]
+    dummy = C.c_void_p(16)
+    assert lib.wl_group_permutation(1, 0, 4, dummy, None) == 1
+    assert lib.wl_group_permutation(1, 1 << 31, 4, dummy, None) == 1
+    assert lib.wl_group_permutation(1, 8, 0, dummy, None) == 1
+    assert lib.wl_group_permutation(1, 8, 4, None, None) == 1
+    lib.wl_version.restype = C.c_char_p
+    assert lib.wl_version() == b"2.0"
