@@ -192,8 +192,11 @@ struct PackedF32Base {
 // Near the axis (w = u^2 < 1/8) the bracket cancels and a degree-3 polynomial in w' replaces br/w'
 // (coefficients: gen_h_poly.py hs 0.125 3, relative error 8e-8).
 // ------------------------------------------------------------------------------------------------------------
-template <int P_, int THREADS_, bool HAS_PHI, int Q_, int MINB_ = 4>
+// SCALAR_ = true (scalar QED, W = cos(phase)): the spin sum is not needed, so the point's
+// sqrt and 2^x are skipped and the reciprocal is that of the nodes alone: 3 MUFU per point-eval at Q = 1.
+template <int P_, int THREADS_, bool HAS_PHI, int Q_, int MINB_ = 4, bool SCALAR_ = false>
 struct Sech2PackedF32 : PackedF32Base<P_, THREADS_, HAS_PHI, Q_, MINB_> {
+    static_assert(!SCALAR_ || Q_ == 1, "the scalar-only variant is compiled for the midpoint rule");
     typedef PackedF32Base<P_, THREADS_, HAS_PHI, Q_, MINB_> B;
     using typename B::Acc;
     using B::NP; using B::NFP; using B::C; using B::iPT; using B::iNODE;
@@ -257,10 +260,13 @@ struct Sech2PackedF32 : PackedF32Base<P_, THREADS_, HAS_PHI, Q_, MINB_> {
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
             // |x_i|^2 and rho_i^2(t_q) (times k^2): eq. (8), (25)-(28)
-            const u64 wp = B::radius2(g, q, v, iPT);
-            float wp0, wp1;
-            upk(wp, wp0, wp1);
-            const u64 Ep = pk(xu_ex2_neg(xu_sqrt_abs(wp0)), xu_ex2_neg(xu_sqrt_abs(wp1)));
+            u64 Ep = 0ull;
+            if constexpr (!SCALAR_) {
+                const u64 wp = B::radius2(g, q, v, iPT);
+                float wp0, wp1;
+                upk(wp, wp0, wp1);
+                Ep = pk(xu_ex2_neg(xu_sqrt_abs(wp0)), xu_ex2_neg(xu_sqrt_abs(wp1)));
+            }
             u64 wm[Q_], rm[Q_], um[Q_], Em[Q_], Dmn[Q_];
 #pragma unroll
             for (int n = 0; n < Q_; ++n) {
@@ -277,8 +283,10 @@ struct Sech2PackedF32 : PackedF32Base<P_, THREADS_, HAS_PHI, Q_, MINB_> {
             }
             const u64 Dp = fma2(Ep, one2, one2);                              //   1 + E_p
             // ONE reciprocal for the point and all nodes; imn[n] = -1/(1 + E_n), ip = 1/(1 + E_p)
-            u64 ip, imn[Q_];
-            if constexpr (Q_ == 1) {
+            u64 ip = 0ull, imn[Q_];
+            if constexpr (SCALAR_) {
+                imn[0] = xu_rcp2(Dmn[0]);                                     // -1/(1+E_m)
+            } else if constexpr (Q_ == 1) {
                 const u64 r = xu_rcp2(mul2(Dp, Dmn[0]));                      // -1/((1+E_p)(1+E_m))
                 ip = mul2(r, Dmn[0]);
                 imn[0] = mul2(r, Dp);
@@ -300,7 +308,7 @@ struct Sech2PackedF32 : PackedF32Base<P_, THREADS_, HAS_PHI, Q_, MINB_> {
                 imn[0] = mul2(t, Dmn[1]);
                 imn[1] = mul2(t, Dmn[0]);
             }
-            acc.sp[q] = fma2(mul2(Ep, ip), ip, acc.sp[q]);                    // E_p/(1+E_p)^2 = sech^2/4
+            if constexpr (!SCALAR_) acc.sp[q] = fma2(mul2(Ep, ip), ip, acc.sp[q]);   // E_p/(1+E_p)^2 = sech^2/4
             u64 gt = g_node(wm[0], rm[0], um[0], Em[0], imn[0]);
             if constexpr (Q_ == 2) gt = add2(gt, g_node(wm[1], rm[1], um[1], Em[1], imn[1]));
             if constexpr (Q_ == 3) {                                          // 5/18 [ g_0 + g_2 + (8/5) g_1 ]

@@ -11,6 +11,7 @@ namespace {
 //   Q = 1: with and without phi_cm, with and without the discretisation estimate
 //   Q = 2, 3: without phi_cm, ordinary evaluation only
 //   the cp.async.bulk staging variant: Q = 1, no phi_cm, ordinary evaluation, P = 4
+//   the scalar-only variant (no spin sum): Q = 1, no phi_cm, ordinary evaluation
 template <int P, int TH>
 cudaError_t launch_shape(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s)
 {
@@ -23,6 +24,9 @@ cudaError_t launch_shape(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s
     if (a.quad == 1) {
         if (phi) return launch_term<Sech2PackedF32<P, TH, true, 1>, false, false>(plan, a, s);
         if (P == 4 && bulk_ok(a)) return launch_term<Sech2PackedF32<4, 256, false, 1>, false, true>(plan, a, s);
+        // scalar loops (W = cos(phase)) in the reducing path: the spin sum is not computed (3 MUFU per point-eval);
+        // the per-loop triage path keeps the full kernel so that its spin output stays meaningful
+        if (a.scalar && !a.phase_out && !a.spin_out) return launch_term<Sech2PackedF32<P, TH, false, 1, 4, true>, false, false>(plan, a, s);
         return launch_term<Sech2PackedF32<P, TH, false, 1>, false, false>(plan, a, s);
     }
     if (phi) return cudaErrorInvalidValue;

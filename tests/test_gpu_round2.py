@@ -151,3 +151,26 @@ def test_grid_validate(api):
         with pytest.raises(api.WLError) as e:
             api.wl_grid_validate(T, rho)
         assert e.value.status == 1
+
+
+@pytest.mark.parametrize("n_T,n_rho", [(64, 64), (12, 40), (16, 16)])
+def test_scalar_only_sech2_kernel_in_every_tile_shape(api, o, n_T, n_rho):
+    """A scalar field in the reducing path runs the packed kernel WITHOUT the spin sum (3 special-function ops per
+    point-eval): against the oracle's W = cos(phase), and consistent with the full kernel's per-loop phases."""
+    n_loops, N, G = 64, 512, 8
+    T, rho = np.geomspace(0.01, 8.0, n_T), np.linspace(0.0, 4.0, n_rho)
+    loops = api.wl_loops_generate(n_loops, N, 91, torch.float32)
+    fs = api.wl_field_create_particle(SECH2, (1.0, 1.0), api.SCALAR)
+    mean, gs = api.wl_eval(fs, loops, dev(T), dev(rho), None, n_groups=G, compute="f32")
+    Wl, ph, _ = api.wl_eval_per_loop(fs, loops, dev(T), dev(rho), None, compute="f32")
+    torch.cuda.synchronize()
+    ref = o.evaluate(SECH2, (1.0, 1.0), loops.cpu().numpy(), T, rho, None, n_groups=G, scalar=True)
+    assert_mean_close(mean.cpu().numpy(), ref["W_mean"], "f32")
+    assert_mean_close(gs.cpu().numpy(), ref["group_sums"], "f32", scale=n_loops // G, what="group sums")
+    # the two kernels round the reciprocal differently: equal to FP32 accuracy, not bit for bit
+    regrouped = Wl.reshape(G, n_loops // G, n_T, n_rho).sum(1)
+    assert float((regrouped - gs).abs().max()) < 2e-4 * (n_loops // G)
+    # a seeded scalar run takes the same kernel: same bits
+    m2, g2 = api.wl_eval_seeded(fs, 91, n_loops, N, dev(T), dev(rho), None, n_groups=G, compute="f32", storage=torch.float32)
+    torch.cuda.synchronize()
+    assert torch.equal(gs, g2)
