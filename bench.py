@@ -317,7 +317,10 @@ def run_ours(args, cfg):
                "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                "ms_per_step": 1e3 * dt / args.steps,
                "call": "wl_eval_host (per rank: its own loops; pinned host memory; wall clock, max over ranks)"}
-        if not np.array_equal(hm, W_mean.cpu().numpy()):
+        # one rank: the same units of loops, hence the same bits; several ranks: the device step is cut like the
+        # whole ensemble (wl_eval_options.ensemble_loops), the host call like its own loops: equal to rounding
+        dm = W_mean.cpu().numpy()
+        if not (np.array_equal(hm, dm) if world == 1 else np.allclose(hm, dm, rtol=1e-12, atol=0)):
             raise SystemExit("bench.py: wl_eval_host and wl_eval disagree")
         del host_loops
 
