@@ -110,6 +110,8 @@ size_t wl_eval_workspace_bytes(int64_t n_loops, int n_ppl, int n_T, int n_rho, i
  * powers of two).  d_T[n_T] > 0; d_rho_cm[n_rho] >= 0; d_phi_cm[n_rho] or NULL
  * (= all zero).  Grid VALUES live on the device and are not read by this call: T <= 0 or a
  * non-finite value gives NaN rows, not an error.  wl_grid_validate checks a host copy.
+ * FP32 range: for the sech^2 and flux-tube profiles with 1e-4 <= lambda <= 1e4 the FP32 kernels carry
+ * squared radii divided by lambda^2; they stay finite while (rho_cm + sqrt(T) |y|)/lambda < 1e18.
  * compute = WL_F64: all arithmetic FP64.  compute = WL_F32: per-term arithmetic
  * FP32 with fast intrinsics, the sums round a loop accumulated in FP64 from
  * FP32 partials of at most 128 terms, cos/cosh and all sums over loops FP64.

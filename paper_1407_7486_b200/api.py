@@ -24,8 +24,13 @@ F32 = 0
 F64 = 1
 
 if not os.path.exists(LIB_PATH):
-    raise ImportError("%s not found: build it with `python -m paper_1407_7486_b200.build` "
-                      "(there is no CPU fallback)" % LIB_PATH)
+    # a fresh checkout (the .so is not in the history): compile the CUDA sources once, in-tree; no CPU fallback
+    try:
+        from . import build as _build
+        _build.build()
+    except Exception as exc:
+        raise ImportError("%s not found and `python -m paper_1407_7486_b200.build` failed (%s): "
+                          "there is no CPU fallback" % (LIB_PATH, exc))
 _lib = C.CDLL(LIB_PATH)
 
 _vp, _dp, _i64, _int, _u64, _sz = C.c_void_p, C.c_void_p, C.c_int64, C.c_int, C.c_uint64, C.c_size_t

@@ -53,6 +53,9 @@ def grids(n_T, n_rho, T_max=6.0, rho_max=3.0, phi=False):
     (UNI, (1.0,), "f64", "f64", 32, 2, 3, 3, 4, False),                 # N = 2: one noise point per loop
     (SECH2, (1.0, 1.0), "f32", "f32", 2048, 64, 64, 64, 4, False),      # units of 2 loops (loops_per_unit > 1)
     (SECH2, (1.0, 1.0), "f32", "f32", 8192, 16, 64, 64, 8, False),      # units of 8 loops
+    (SECH2, (1.0, 1.0), "f32", "f32", 4, 65536, 8, 40, 2, False),       # the longest loop: skeleton of 64 points
+    (SECH2, (1.0, 1.0), "f64", "f64", 2, 65536, 4, 40, 2, False),       # ... of 128 points (chunks of 512)
+    (FLUX, (10.0, 1.0), "f64", "f32", 4, 16384, 4, 40, 2, False),       # generic FP64 kernel: chunks of 256, skeleton of 64
 ])
 def test_seeded_equals_generate_then_eval_bit_for_bit(api, profile, params, compute, storage, n_loops, N, nT, nr, G, phi):
     T, rho, ph = grids(nT, nr, phi=phi)

@@ -69,7 +69,7 @@ def run_gpu(api, cfg, loops, T, rho, phi, G, compute):
 # --------------------------------------------------------------------------- generator (a0)
 
 def test_generator_matches_the_oracle_twin(api, o):
-    for (n, N, seed) in ((64, 256, 1), (5, 2, 7), (3, 8192, 4), (33, 1024, 2)):
+    for (n, N, seed) in ((64, 256, 1), (5, 2, 7), (3, 8192, 4), (33, 1024, 2), (3, 16384, 5), (2, 65536, 11), (7, 4, 6)):
         y = api.wl_loops_generate(n, N, seed, torch.float64)
         torch.cuda.synchronize()
         ref = o.generate_loops(seed, n, N)
