@@ -8,6 +8,8 @@ in w and reports the maximum relative error on a fine grid.
 
 Usage:  python gen_h_poly.py <w_max> <degree>          h(w) on [0, w_max]
         python gen_h_poly.py L <degree>                1 - log2(1+E) on E in [0, 1] (absolute error)
+        python gen_h_poly.py Lw <w_min> <degree>       the same on E in [0, 1.001 * 2^-sqrt(w_min)]: the range of E = 2^(-u') when
+                                                       u'^2 >= w_min (the "far block" tiers of wl_terms_packed_f32.cuh)
         python gen_h_poly.py E2 <degree>               2^(-f) on f in [-1/2, 1/2] (relative error)
         python gen_h_poly.py hs <w_max> <degree>       h rescaled for the packed FP32 / lean FP64 kernels:
                                                        h(w)/(4 log2 e) as a polynomial in w' = 4 (log2 e)^2 w
@@ -82,6 +84,15 @@ if __name__ == "__main__":
               % (mp.nstr(max_abs_err(coef, 1, L, lambda c: c), 3), mp.nstr(max_abs_err(coef, 1, L, f32), 3)))
         for i, c in enumerate(coef):
             print("c%d = %s" % (i, mp.nstr(c, 20)))
+        sys.exit(0)
+    if sys.argv[1] == "Lw":
+        w_min, deg = float(sys.argv[2]), int(sys.argv[3])
+        e_max = mp.power(2, -mp.sqrt(w_min)) * mp.mpf("1.001")
+        coef = fit(e_max, deg, L)
+        print("// 1 - log2(1+E), E in [0, %s] (u'^2 >= %g), degree %d" % (mp.nstr(e_max, 8), w_min, deg))
+        print("// max abs. error: exact coefficients %s, float32 coefficients %s"
+              % (mp.nstr(max_abs_err(coef, e_max, L, lambda c: c), 3), mp.nstr(max_abs_err(coef, e_max, L, f32), 3)))
+        print("{ " + ", ".join("%sf" % mp.nstr(c, 12) for c in coef) + " }")
         sys.exit(0)
     if sys.argv[1] == "E2":
         deg = int(sys.argv[2])

@@ -13,8 +13,9 @@
 // one LDS.64 (shared-memory loads return through the same queue as the special-function results: every
 // 4 bytes per lane cost about one XU-pipe clock, profiles/r01_pipe_rates.md); (iii) the special-function
 // count per point-eval of the sech^2 profile is 3 + 2Q (Q = Gauss-Legendre points of eq. (24); 5 at Q = 1):
-//       sqrt(|x_i|^2), 2^(-u_p), [rsqrt(rho_i^2(t_q)), 2^(-u_q)] x Q, ONE reciprocal 1/((1+E_p) prod_q (1+E_q))
-//   and log2(1+E_q) is a degree-8 polynomial in E_q in [0,1] on the FMA pipe.
+//       sqrt(|x_i|^2), 2^(-u_p), [rsqrt(rho_i^2(t_q)), 2^(-u_q)] x Q, and ONE reciprocal per staged point and THREAD
+//   (the product of the denominators (1+E_p) prod_q (1+E_q) of all P grid points is inverted once), i.e. 2 + 2Q + 1/P;
+//   log2(1+E_q) is a degree-8 polynomial in E_q in [0,1] on the FMA pipe.
 //
 // Staged record of a point i (floats; C = 2 values per position without phi_cm, 3 with):
 //     [ y_x, (y_y), |y|^2 ]  [ y(t_q)_x, (y(t_q)_y), |y(t_q)|^2 ] x Q  [ dy_y/2, (dy_x/2), y_i x y_{i+1} ]
@@ -221,23 +222,127 @@ struct Sech2PackedF32 : PackedF32Base<P_, THREADS_, HAS_PHI, Q_, MINB_> {
     }
     __device__ double b_scale() const { return 4.0 * eB0; }
 
-    // g-term of one node from (w' clamped, 1/sqrt(w'), u', E, -1/(1+E)):  br/w' or the near-axis polynomial
+    // ---- far blocks --------------------------------------------------------------------------------------------
+    // The near-axis polynomial, its select and the guard of rsqrt are needed only where a node can come within
+    // u^2 < 1/8 of the axis.  While staging, every warp records the bounding box of the 32 segments it stages
+    // (unit-loop coordinates); before a block of kSumBlock = 128 staged points is walked, every thread bounds
+    // rho_i^2(t) from below for its P grid points over the block's box, and if the whole WARP is clear of the axis
+    // the block runs an instantiation without those instructions.  The same bound limits E = 2^(-u') from above, and on
+    // a shorter range of E the polynomial for 1 - log2(1+E) reaches the same 6e-8 with a lower degree: kTiers
+    // instantiations of the walk, the tier being a function of the loop, the grid and the tile shape only.
+    static constexpr bool kBlockBounds = true;
+    static constexpr int kBoundsBlocks = B::kChunk / B::kSumBlock, kBoundsSlots = B::kSumBlock / 32;
+    static_assert(B::kSumBlock % 32 == 0 && B::kChunk % B::kSumBlock == 0, "a warp's 32 staged points lie in one block");
+    __host__ __device__ static constexpr size_t stage_bytes(int q) { return B::stage_bytes(q) + sizeof(float4) * kBoundsBlocks * kBoundsSlots; }
+
+    __device__ __forceinline__ static int ordered(float f) { const int i = __float_as_int(f); return i ^ ((i >> 31) & 0x7fffffff); }
+    __device__ __forceinline__ static float unordered(int i) { return __int_as_float(i ^ ((i >> 31) & 0x7fffffff)); }
+
+    // every thread of the CTA, once per staging step: ib = first staged index of the step, (y, z) = its segment
+    __device__ __forceinline__ void note_bounds(unsigned char* s, int ib, bool valid, double yx, double yy, double zx, double zy) const
+    {
+        const float inf = __int_as_float(0x7f800000);
+        const float x0 = valid ? fminf(float(yx), float(zx)) : inf, x1 = valid ? fmaxf(float(yx), float(zx)) : -inf;
+        const float y0 = valid ? fminf(float(yy), float(zy)) : inf, y1 = valid ? fmaxf(float(yy), float(zy)) : -inf;
+        const float bx0 = unordered(__reduce_min_sync(0xffffffffu, ordered(x0))), bx1 = unordered(__reduce_max_sync(0xffffffffu, ordered(x1)));
+        const float by0 = unordered(__reduce_min_sync(0xffffffffu, ordered(y0))), by1 = unordered(__reduce_max_sync(0xffffffffu, ordered(y1)));
+        const int i0 = ib + (int)(threadIdx.x & ~31u);                 // first staged index of this warp's 32 points
+        if ((threadIdx.x & 31u) == 0 && i0 < B::kChunk)
+            reinterpret_cast<float4*>(s + B::stage_bytes(0))[i0 / 32] = make_float4(bx0, bx1, by0, by1);
+    }
+
+    // Tier of the block starting at staged index i0 = how far from the axis every node of the block stays for every grid
+    // point of this WARP: a lower bound of w' (conservative: the box bounds every point of every segment, the margins
+    // cover the FP32 rounding of w' and of this test) is compared with kTierW[].  Tier 0: the axis may be near.
+    static constexpr int kTiers = 6;
+    __device__ __forceinline__ static int block_tier(const unsigned char* s, int i0, const Grid& g)
+    {
+        const float4* bb = reinterpret_cast<const float4*>(s + B::stage_bytes(0)) + (i0 / B::kSumBlock) * kBoundsSlots;
+        float4 b = bb[0];
+#pragma unroll
+        for (int k = 1; k < kBoundsSlots; ++k) {
+            const float4 c = bb[k];
+            b.x = fminf(b.x, c.x); b.y = fmaxf(b.y, c.y); b.z = fminf(b.z, c.z); b.w = fmaxf(b.w, c.w);
+        }
+        const float ext2 = fmaxf(b.x * b.x, b.y * b.y) + fmaxf(b.z * b.z, b.w * b.w);   // max |y|^2 over the box
+        float wlow = 1e30f;
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+            float R2[2], ax[2], Tt[2], ay[2] = {0.0f, 0.0f};
+            upk(g.R2[q], R2[0], R2[1]);
+            upk(g.ax[q], ax[0], ax[1]);
+            upk(g.Tt[q], Tt[0], Tt[1]);
+            if (HAS_PHI) upk(g.ay[q], ay[0], ay[1]);
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                // k x_cm = (ax, ay)/(2 k sqrt T), k sqrt(T) = sqrt(Tt): the node is k x_cm + k sqrt(T) y, y in the box
+                const float t = xu_rsqrt(Tt[h]), ks = Tt[h] * t, cx = 0.5f * ax[h] * t, cy = 0.5f * ay[h] * t;
+                const float dx = fmaxf(fmaxf(fmaf(ks, b.x, cx), -fmaf(ks, b.y, cx)), 0.0f);
+                const float dy = fmaxf(fmaxf(fmaf(ks, b.z, cy), -fmaf(ks, b.w, cy)), 0.0f);
+                const float d2 = fmaf(dx, dx, dy * dy);
+                const float w = fmaf(d2, 0.999f, -1e-5f * fmaf(Tt[h], ext2, R2[h]));
+                wlow = (w >= 0.0f) ? fminf(wlow, w) : 0.0f;                   // a NaN counts as "near"
+            }
+        }
+        // non-negative floats order like their bit patterns
+        const float wwarp = __int_as_float(__reduce_min_sync(0xffffffffu, __float_as_int(wlow)));
+        int tier = 0;
+#pragma unroll
+        for (int k = 1; k < kTiers; ++k) tier = (wwarp >= tier_w(k)) ? k : tier;
+        return tier;
+    }
+    // tier k > 0 holds when w' >= tier_w(k) for every node: E = 2^(-u') <= 2^(-sqrt(tier_w)), and 1 - log2(1+E) needs
+    // only degree tier_deg(k) there for the same 6e-8 (gen_h_poly.py Lw <tier_w> <degree>)
+    __host__ __device__ static constexpr float tier_w(int k) { return k == 1 ? 1.05f : k == 2 ? 9.0f : k == 3 ? 16.0f : k == 4 ? 36.0f : 144.0f; }
+    __host__ __device__ static constexpr int tier_deg(int k) { return k == 0 ? 8 : k == 1 ? 6 : k == 2 ? 4 : k == 3 ? 3 : k == 4 ? 2 : 1; }
+    __host__ __device__ static constexpr float tier_coef(int k, int i)
+    {
+        constexpr float c0[9] = {0.999999943578f, -1.44268585129f, 0.721095768202f, -0.478176441505f, 0.345429336575f,
+                                 -0.238041983614f, 0.13314692741f, -0.0494333683912f, 0.00866569930832f};   // L 8
+        constexpr float c1[7] = {0.999999951917f, -1.44268542229f, 0.72102782158f, -0.476826061169f, 0.33512281736f,
+                                 -0.20083019495f, 0.0676755895834f};                                            // Lw 1.05 6
+        constexpr float c2[5] = {0.999999986538f, -1.44268965027f, 0.720999117524f, -0.472913355165f, 0.283761002847f};  // Lw 9 4
+        constexpr float c3[4] = {0.999999960862f, -1.44267499105f, 0.719731652215f, -0.438694041338f};         // Lw 16 3
+        constexpr float c4[3] = {0.999999943498f, -1.44262997327f, 0.710212211046f};                           // Lw 36 2
+        constexpr float c5[2] = {0.999999994616f, -1.44251877967f};                                            // Lw 144 1
+        return k == 0 ? c0[i] : k == 1 ? c1[i] : k == 2 ? c2[i] : k == 3 ? c3[i] : k == 4 ? c4[i] : c5[i];
+    }
+
+    // 1/den[q] for every pair from ONE special-function reciprocal per thread: the product of all 2 NP lanes'
+    // denominators is inverted once and each lane's inverse is recovered by multiplying the others back in
+    // (every denominator is a product of at most four factors in [1, 2], so the product of all stays below 2^16).
+    __device__ __forceinline__ static void shared_inverse(const u64 (&den)[NP], u64 (&inv)[NP])
+    {
+        static_assert(NP <= 2, "written for one or two register pairs");
+        if constexpr (NP == 1) {
+            float a, b;
+            upk(den[0], a, b);
+            const float r = xu_rcp(a * b);
+            inv[0] = pk(r * b, r * a);
+        } else {
+            float a, b;
+            upk(mul2(den[0], den[1]), a, b);
+            const float r = xu_rcp(a * b);
+            const u64 iq = pk(r * b, r * a);
+            inv[0] = mul2(iq, den[1]);
+            inv[1] = mul2(iq, den[0]);
+        }
+    }
+
+    // g-term of one node from (w' clamped, 1/sqrt(w'), u', E, -1/(1+E)):  br/w' or, in tier 0, the near-axis polynomial
+    template <int TIER>
     __device__ __forceinline__ static u64 g_node(u64 wm, u64 rm, u64 um, u64 Em, u64 imn)
     {
         constexpr float kPolyBelow = 1.0406844905f;     // w' < this  <=>  u^2 < 1/8
-        // 1 - log2(1+E), E in [0,1]: gen_h_poly.py L 8, abs. error 6e-8
-        u64 L = pk1(0.00866569930832f);
-        L = fma2(L, Em, pk1(-0.0494333683912f));
-        L = fma2(L, Em, pk1(0.13314692741f));
-        L = fma2(L, Em, pk1(-0.238041983614f));
-        L = fma2(L, Em, pk1(0.345429336575f));
-        L = fma2(L, Em, pk1(-0.478176441505f));
-        L = fma2(L, Em, pk1(0.721095768202f));
-        L = fma2(L, Em, pk1(-1.44268585129f));
-        // last Horner step folded with the second term: 1 - log2(1+E) = c0 + E L'(E) and
-        // -u' E/(1+E) = E (u' imn), so br = c0 + E (L' + u' imn): one instruction fewer
-        const u64 br = fma2(fma2(um, imn, L), Em, pk1(0.999999943578f));       // (1 - log2(1+E)) - u' E/(1+E)
+        // 1 - log2(1+E) = c0 + E L'(E), abs. error 6e-8 on the tier's range of E
+        constexpr int D = tier_deg(TIER);
+        u64 L = pk1(tier_coef(TIER, D));
+#pragma unroll
+        for (int k = D - 1; k >= 1; --k) L = fma2(L, Em, pk1(tier_coef(TIER, k)));
+        // last Horner step folded with the second term: -u' E/(1+E) = E (u' imn), so br = c0 + E (L' + u' imn)
+        const u64 br = fma2(fma2(um, imn, L), Em, pk1(tier_coef(TIER, 0)));    // (1 - log2(1+E)) - u' E/(1+E)
         const u64 hE = mul2(br, mul2(rm, rm));                                  // br / w'
+        if constexpr (TIER > 0) return hE;
         // h(w)/(4 log2 e) in w' (gen_h_poly.py hs 0.125 3, rel. error 8e-8)
         u64 hP = fma2(pk1(-1.2801479229129e-5f), wm, pk1(0.00027690498335525f));
         hP = fma2(hP, wm, pk1(-0.0052033291295960f));
@@ -249,6 +354,7 @@ struct Sech2PackedF32 : PackedF32Base<P_, THREADS_, HAS_PHI, Q_, MINB_> {
         return pk(wm0 < kPolyBelow ? hP0 : hE0, wm1 < kPolyBelow ? hP1 : hE1);
     }
 
+    template <int TIER = 0>
     __device__ __forceinline__ void point(const unsigned char* s, int i, const Grid& g, Acc& acc) const
     {
         // one LDS.128 + one LDS.64 per staged point at Q = 1 (a broadcast: every lane reads the same address);
@@ -257,65 +363,90 @@ struct Sech2PackedF32 : PackedF32Base<P_, THREADS_, HAS_PHI, Q_, MINB_> {
         B::load_record(s, i, v);
         const u64 one2 = pk1(1.0f), mone2 = pk1(-1.0f);
         constexpr float kTiny = 1e-36f;                 // rsqrt(kTiny)^2 is still finite
+        u64 Ep[NP], Dp[NP], wm[NP][Q_], rm[NP][Q_], um[NP][Q_], Em[NP][Q_], Dmn[NP][Q_], den[NP], inv[NP], PD[NP], D01[NP];
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
             // |x_i|^2 and rho_i^2(t_q) (times k^2): eq. (8), (25)-(28)
-            u64 Ep = 0ull;
+            Ep[q] = 0ull;
             if constexpr (!SCALAR_) {
-                const u64 wp = B::radius2(g, q, v, iPT);
                 float wp0, wp1;
-                upk(wp, wp0, wp1);
-                Ep = pk(xu_ex2_neg(xu_sqrt_abs(wp0)), xu_ex2_neg(xu_sqrt_abs(wp1)));
+                upk(B::radius2(g, q, v, iPT), wp0, wp1);
+                Ep[q] = pk(xu_ex2_neg(xu_sqrt_abs(wp0)), xu_ex2_neg(xu_sqrt_abs(wp1)));
             }
-            u64 wm[Q_], rm[Q_], um[Q_], Em[Q_], Dmn[Q_];
 #pragma unroll
             for (int n = 0; n < Q_; ++n) {
                 float w0, w1, u0, u1;
                 upk(B::radius2(g, q, v, iNODE + C * n), w0, w1);
-                w0 = fmaxf(w0, kTiny);
-                w1 = fmaxf(w1, kTiny);
-                wm[n] = pk(w0, w1);
-                rm[n] = pk(xu_rsqrt(w0), xu_rsqrt(w1));
-                um[n] = mul2(wm[n], rm[n]);                                   // u' = sqrt(w')
-                upk(um[n], u0, u1);
-                Em[n] = pk(xu_ex2_neg(u0), xu_ex2_neg(u1));
-                Dmn[n] = fma2(Em[n], mone2, mone2);                           // -(1 + E_q)
+                if constexpr (TIER == 0) {
+                    w0 = fmaxf(w0, kTiny);
+                    w1 = fmaxf(w1, kTiny);
+                }
+                wm[q][n] = pk(w0, w1);
+                rm[q][n] = pk(xu_rsqrt(w0), xu_rsqrt(w1));
+                um[q][n] = mul2(wm[q][n], rm[q][n]);                          // u' = sqrt(w')
+                upk(um[q][n], u0, u1);
+                Em[q][n] = pk(xu_ex2_neg(u0), xu_ex2_neg(u1));
+                Dmn[q][n] = fma2(Em[q][n], mone2, mone2);                     // -(1 + E_q)
             }
-            const u64 Dp = fma2(Ep, one2, one2);                              //   1 + E_p
-            // ONE reciprocal for the point and all nodes; imn[n] = -1/(1 + E_n), ip = 1/(1 + E_p)
+            Dp[q] = fma2(Ep[q], one2, one2);                                  //   1 + E_p
+            // the denominator the point and all nodes share
+            if constexpr (SCALAR_) den[q] = Dmn[q][0];
+            else if constexpr (Q_ == 1) den[q] = mul2(Dp[q], Dmn[q][0]);
+            else if constexpr (Q_ == 2) { PD[q] = mul2(Dmn[q][0], Dmn[q][1]); den[q] = mul2(Dp[q], PD[q]); }
+            else { D01[q] = mul2(Dmn[q][0], Dmn[q][1]); PD[q] = mul2(D01[q], Dmn[q][2]); den[q] = mul2(Dp[q], PD[q]); }
+        }
+        shared_inverse(den, inv);                                             // ONE reciprocal per staged point and thread
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+            // imn[n] = -1/(1 + E_n), ip = 1/(1 + E_p)
+            const u64 r = inv[q];
             u64 ip = 0ull, imn[Q_];
             if constexpr (SCALAR_) {
-                imn[0] = xu_rcp2(Dmn[0]);                                     // -1/(1+E_m)
+                imn[0] = r;                                                   // -1/(1+E_m)
             } else if constexpr (Q_ == 1) {
-                const u64 r = xu_rcp2(mul2(Dp, Dmn[0]));                      // -1/((1+E_p)(1+E_m))
-                ip = mul2(r, Dmn[0]);
-                imn[0] = mul2(r, Dp);
+                ip = mul2(r, Dmn[q][0]);                                      // r = -1/((1+E_p)(1+E_m))
+                imn[0] = mul2(r, Dp[q]);
             } else if constexpr (Q_ == 2) {
-                const u64 PD = mul2(Dmn[0], Dmn[1]);                          // (+)
-                const u64 r = xu_rcp2(mul2(Dp, PD));                          // (+)
-                ip = mul2(r, PD);
-                const u64 rDp = mul2(r, Dp);
-                imn[0] = mul2(rDp, Dmn[1]);
-                imn[1] = mul2(rDp, Dmn[0]);
+                ip = mul2(r, PD[q]);                                          // r, PD (+)
+                const u64 rDp = mul2(r, Dp[q]);
+                imn[0] = mul2(rDp, Dmn[q][1]);
+                imn[1] = mul2(rDp, Dmn[q][0]);
             } else {
-                const u64 D01 = mul2(Dmn[0], Dmn[1]);                         // (+)
-                const u64 PD = mul2(D01, Dmn[2]);                             // (-)
-                const u64 r = xu_rcp2(mul2(Dp, PD));                          // (-)
-                ip = mul2(r, PD);                                             // (+)
-                const u64 rDp = mul2(r, Dp);                                  // (-)
-                imn[2] = mul2(rDp, D01);                                      // (-)
-                const u64 t = mul2(rDp, Dmn[2]);                              // (+)
-                imn[0] = mul2(t, Dmn[1]);
-                imn[1] = mul2(t, Dmn[0]);
+                ip = mul2(r, PD[q]);                                          // r, PD (-); D01 (+)
+                const u64 rDp = mul2(r, Dp[q]);                               // (-)
+                imn[2] = mul2(rDp, D01[q]);                                   // (-)
+                const u64 t = mul2(rDp, Dmn[q][2]);                           // (+)
+                imn[0] = mul2(t, Dmn[q][1]);
+                imn[1] = mul2(t, Dmn[q][0]);
             }
-            if constexpr (!SCALAR_) acc.sp[q] = fma2(mul2(Ep, ip), ip, acc.sp[q]);   // E_p/(1+E_p)^2 = sech^2/4
-            u64 gt = g_node(wm[0], rm[0], um[0], Em[0], imn[0]);
-            if constexpr (Q_ == 2) gt = add2(gt, g_node(wm[1], rm[1], um[1], Em[1], imn[1]));
+            if constexpr (!SCALAR_) acc.sp[q] = fma2(mul2(Ep[q], ip), ip, acc.sp[q]);   // E_p/(1+E_p)^2 = sech^2/4
+            u64 gt = g_node<TIER>(wm[q][0], rm[q][0], um[q][0], Em[q][0], imn[0]);
+            if constexpr (Q_ == 2) gt = add2(gt, g_node<TIER>(wm[q][1], rm[q][1], um[q][1], Em[q][1], imn[1]));
             if constexpr (Q_ == 3) {                                          // 5/18 [ g_0 + g_2 + (8/5) g_1 ]
-                gt = add2(gt, g_node(wm[2], rm[2], um[2], Em[2], imn[2]));
-                gt = fma2(g_node(wm[1], rm[1], um[1], Em[1], imn[1]), pk1(1.6f), gt);
+                gt = add2(gt, g_node<TIER>(wm[q][2], rm[q][2], um[q][2], Em[q][2], imn[2]));
+                gt = fma2(g_node<TIER>(wm[q][1], rm[q][1], um[q][1], Em[q][1], imn[1]), pk1(1.6f), gt);
             }
             acc.add_phase(q, gt, v);
+        }
+    }
+
+    template <int TIER>
+    __device__ __forceinline__ void walk(const unsigned char* s, int i0, int ie, const Grid& g, Acc& acc) const
+    {
+#pragma unroll B::kUnroll
+        for (int i = i0; i < ie; ++i) point<TIER>(s, i, g, acc);
+    }
+    // one block of at most kSumBlock staged points, [i0, ie)
+    __device__ __forceinline__ void block(const unsigned char* s, int i0, int ie, const Grid& g, Acc& acc) const
+    {
+        const int tier = block_tier(s, i0, g);
+        switch (tier) {
+            case 0: walk<0>(s, i0, ie, g, acc); break;
+            case 1: walk<1>(s, i0, ie, g, acc); break;
+            case 2: walk<2>(s, i0, ie, g, acc); break;
+            case 3: walk<3>(s, i0, ie, g, acc); break;
+            case 4: walk<4>(s, i0, ie, g, acc); break;
+            default: walk<5>(s, i0, ie, g, acc); break;
         }
     }
 };

@@ -22,6 +22,11 @@
 //   void stage(smem, i, yx, yy, zx, zy)                       derive and store point i (y) and its neighbour (z)
 //   void point(smem, i, grid, acc)                            add staged point i to the sums of all P grid points
 //   double g_scale(), b_scale()                               constant factors of phase and spin
+// Optional (a Term that declares kBlockBounds = true; needs kSumBlock > 0):
+//   void note_bounds(smem, ib, valid, yx, yy, zx, zy)         called by EVERY thread next to stage(): the Term keeps a
+//                                                             bounding box of every block of kSumBlock staged segments
+//   void block(smem, i0, ie, grid, acc)                       walks the block [i0, ie) itself instead of point() calls
+//                                                             (it may pick a cheaper code path for the whole warp)
 //
 // Algebra (eq. (8), (21)-(28)), with c = x_cm, s = sqrt(T), unit-loop point y_i,
 // node y_i(t) = y_i + t (y_{i+1} - y_i) (t = 1/2: the midpoint), step dy_i = y_{i+1} - y_i:
@@ -89,6 +94,11 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
+template <class T, class = void> struct term_block_bounds { static constexpr bool value = false; };
+template <class T> struct term_block_bounds<T, decltype((void)T::kBlockBounds)> { static constexpr bool value = T::kBlockBounds; };
+
+constexpr int kRhoStrip = 8;     // width in rho_cm of the strips the grid is walked in (wilson_body)
+
 // Shared memory a launch needs beyond the staged chunk.
 template <class Term>
 __host__ __device__ inline size_t wilson_extra_smem(int n_ppl, bool seeded, bool bulk, bool loops_are_f64)
@@ -118,19 +128,33 @@ __device__ __forceinline__ void wilson_body(const EvalArgs& a, const int n_grid,
     const Term term(a);
 
     // ---- per-thread grid-point constants (FP64 on the way in, then the Term's compute type) ----
+    // Which grid points a thread owns.  The grid is walked in strips of kRhoStrip = 8 neighbouring rho_cm: within a strip
+    // rho runs fastest, then the proper time, so that 128 consecutive positions v are a compact patch of 16 proper
+    // times x 8 rho_cm (the last strip may be narrower).  With v = ((tile * warps + warp) * P + j) * 32 + lane a warp
+    // owns one such patch and the P points of a thread share rho_cm: the whole warp sees the flux tube's axis from
+    // about one distance at about one loop size, which is what lets a Term choose one code path for all of its lanes
+    // (wl_terms_packed_f32.cuh, "far blocks").  gp[j] = t * n_rho + r is the point's index in every output array.
     typename Term::Grid grid;
     int gp[P];
+    unsigned gp_ok = 0;
     {
         double Tj[P], rj[P], cxj[P], cyj[P];
 #pragma unroll
         for (int j = 0; j < P; ++j) {
-            gp[j] = tile * (THREADS * P) + j * THREADS + tid;
-            const int g = min(gp[j], n_grid - 1);
-            Tj[j] = a.T[g / a.n_rho];
-            rj[j] = a.rho[g % a.n_rho];
+            const int v = ((tile * (THREADS / 32) + (tid >> 5)) * P + j) * 32 + (tid & 31);
+            if (v < n_grid) gp_ok |= 1u << j;
+            const int vc = min(v, n_grid - 1);
+            constexpr int RB = kRhoStrip;
+            const int nb = a.n_rho / RB, rem = a.n_rho % RB, full = nb * RB * a.n_T;
+            int it, ir;
+            if (vc < full) { const int blk = vc / (RB * a.n_T), w = vc % (RB * a.n_T); it = w / RB; ir = blk * RB + w % RB; }
+            else { const int w = vc - full; it = w / rem; ir = nb * RB + w % rem; }
+            gp[j] = it * a.n_rho + ir;
+            Tj[j] = a.T[it];
+            rj[j] = a.rho[ir];
             cxj[j] = rj[j];
             cyj[j] = 0.0;
-            if (Term::kHasPhi) { const double ph = a.phi[g % a.n_rho]; cxj[j] = rj[j] * cos(ph); cyj[j] = rj[j] * sin(ph); }
+            if (Term::kHasPhi) { const double ph = a.phi[ir]; cxj[j] = rj[j] * cos(ph); cyj[j] = rj[j] * sin(ph); }
         }
         grid.load(term, Tj, rj, cxj, cyj);
     }
@@ -212,38 +236,43 @@ __device__ __forceinline__ void wilson_body(const EvalArgs& a, const int n_grid,
                 if (seeded) dloop_chunk(a.seed, (uint64_t)(a.loop_begin + loop), shp, c0 / CHUNK, sc->skel, yraw);
                 const unsigned char* ring = sRing + (size_t)(ring_idx & 1) * (CHUNK + 2) * raw_elem;
                 if (BULK) mbar_wait(sBar + (ring_idx & 1), (uint32_t)((ring_idx >> 1) & 1));
-                for (int i = tid; i < cn; i += THREADS) {     // stage: derived unit-loop quantities, FP64
-                    double yx, yy, zx, zy;
-                    if (BULK) {
-                        if (a.loops_are_f64) {
-                            const double2 u = reinterpret_cast<const double2*>(ring)[i], v = reinterpret_cast<const double2*>(ring)[i + 1];
-                            yx = u.x; yy = u.y; zx = v.x; zy = v.y;
+                for (int ib = 0; ib < cn; ib += THREADS) {    // stage: derived unit-loop quantities, FP64
+                    const int i = ib + tid;
+                    const bool valid = i < cn;
+                    double yx = 0.0, yy = 0.0, zx = 0.0, zy = 0.0;
+                    if (valid) {
+                        if (BULK) {
+                            if (a.loops_are_f64) {
+                                const double2 u = reinterpret_cast<const double2*>(ring)[i], v = reinterpret_cast<const double2*>(ring)[i + 1];
+                                yx = u.x; yy = u.y; zx = v.x; zy = v.y;
+                            } else {
+                                const float2 u = reinterpret_cast<const float2*>(ring)[i], v = reinterpret_cast<const float2*>(ring)[i + 1];
+                                yx = u.x; yy = u.y; zx = v.x; zy = v.y;
+                            }
+                        } else if (seeded) {
+                            // what wl_loops_generate stores: y - centre of mass, rounded once to the storage type
+                            const double2 u = yraw[i], v = yraw[i + 1], m = sc->mean;
+                            yx = u.x - m.x; yy = u.y - m.y; zx = v.x - m.x; zy = v.y - m.y;
+                            if (!a.loops_are_f64) { yx = (double)(float)yx; yy = (double)(float)yy; zx = (double)(float)zx; zy = (double)(float)zy; }
                         } else {
-                            const float2 u = reinterpret_cast<const float2*>(ring)[i], v = reinterpret_cast<const float2*>(ring)[i + 1];
-                            yx = u.x; yy = u.y; zx = v.x; zy = v.y;
+                            int n = c0 + i;
+                            int n1 = (n + 1 == N) ? 0 : n + 1;    // closed loop, i+1 mod N
+                            if (DISC) {                           // sub-worldline: every 2nd / 4th point, closed on itself
+                                n = pass + 2 * (c0 + i);
+                                n1 = n + (pass ? 4 : 2);
+                                if (n1 >= N) n1 -= N;
+                            }
+                            if (a.loops_are_f64) {
+                                const double2 u = L64[n], v = L64[n1];
+                                yx = u.x; yy = u.y; zx = v.x; zy = v.y;
+                            } else {
+                                const float2 u = L32[n], v = L32[n1];
+                                yx = u.x; yy = u.y; zx = v.x; zy = v.y;
+                            }
                         }
-                    } else if (seeded) {
-                        // what wl_loops_generate stores: y - centre of mass, rounded once to the storage type
-                        const double2 u = yraw[i], v = yraw[i + 1], m = sc->mean;
-                        yx = u.x - m.x; yy = u.y - m.y; zx = v.x - m.x; zy = v.y - m.y;
-                        if (!a.loops_are_f64) { yx = (double)(float)yx; yy = (double)(float)yy; zx = (double)(float)zx; zy = (double)(float)zy; }
-                    } else {
-                        int n = c0 + i;
-                        int n1 = (n + 1 == N) ? 0 : n + 1;    // closed loop, i+1 mod N
-                        if (DISC) {                           // sub-worldline: every 2nd / 4th point, closed on itself
-                            n = pass + 2 * (c0 + i);
-                            n1 = n + (pass ? 4 : 2);
-                            if (n1 >= N) n1 -= N;
-                        }
-                        if (a.loops_are_f64) {
-                            const double2 u = L64[n], v = L64[n1];
-                            yx = u.x; yy = u.y; zx = v.x; zy = v.y;
-                        } else {
-                            const float2 u = L32[n], v = L32[n1];
-                            yx = u.x; yy = u.y; zx = v.x; zy = v.y;
-                        }
+                        term.stage(sStaged, i, yx, yy, zx, zy);
                     }
-                    term.stage(sStaged, i, yx, yy, zx, zy);
+                    if constexpr (term_block_bounds<Term>::value) term.note_bounds(sStaged, ib, valid, yx, yy, zx, zy);
                 }
                 __syncthreads();
                 if (BULK) {                                   // slot (ring_idx + 1) & 1 was last read one chunk ago
@@ -255,8 +284,12 @@ __device__ __forceinline__ void wilson_body(const EvalArgs& a, const int n_grid,
                     for (int i0 = 0; i0 < cn; i0 += (SB > 0 ? SB : 1)) {
                         acc.zero();
                         const int ie = min(i0 + SB, cn);
+                        if constexpr (term_block_bounds<Term>::value) {
+                            term.block(sStaged, i0, ie, grid, acc);
+                        } else {
 #pragma unroll Term::kUnroll
-                        for (int i = i0; i < ie; ++i) term.point(sStaged, i, grid, acc);
+                            for (int i = i0; i < ie; ++i) term.point(sStaged, i, grid, acc);
+                        }
                         acc.flush(grid, dph, dsp);
                     }
                 } else {
@@ -271,14 +304,13 @@ __device__ __forceinline__ void wilson_body(const EvalArgs& a, const int n_grid,
         const double g_scale = term.g_scale(), b_scale = term.b_scale();
 #pragma unroll
         for (int j = 0; j < P; ++j) {
-            const int g = min(gp[j], n_grid - 1);
-            const double T = a.T[g / a.n_rho];
+            const double T = a.T[gp[j] / a.n_rho];
             if (!DISC) {
                 const double phase = g_scale * dph[j];
                 const double spin = b_scale * (T / double(N)) * dsp[j];
                 const double W = a.scalar ? cos(phase) : cos(phase) * cosh(spin);
                 Wsum[0][j] += W;
-                if (gp[j] < n_grid) {
+                if (gp_ok >> j & 1) {
                     if (a.phase_out) a.phase_out[loop * n_grid + gp[j]] = phase;
                     if (a.spin_out) a.spin_out[loop * n_grid + gp[j]] = spin;
                 }
@@ -296,7 +328,7 @@ __device__ __forceinline__ void wilson_body(const EvalArgs& a, const int n_grid,
     for (int v = 0; v < kLevels; ++v)
 #pragma unroll
         for (int j = 0; j < P; ++j)
-            if (gp[j] < n_grid) a.partial[((int64_t)v * n_units + unit) * n_grid + gp[j]] = Wsum[v][j];
+            if (gp_ok >> j & 1) a.partial[((int64_t)v * n_units + unit) * n_grid + gp[j]] = Wsum[v][j];
 }
 
 template <class Term, bool DISC, bool BULK>
