@@ -52,7 +52,8 @@ SM_COUNT = 148
 ISSUE_LANES_PER_CLK_SM = 128      # 4 sub-partitions x 1 warp instruction (32 lanes) per clock
 FP64_LANES_PER_CLK_SM = 64        # measured 63.8 (profiles/r01_pipe_rates.md)
 SFU_LANES_PER_CLK_SM = 16         # measured 15.9
-KERNEL_SFU_OPS = 5                # MUFU per point-eval in k_wilson<Sech2PackedF32> at Q = 1 (sqrt, rsqrt, 2 x ex2, rcp); + 2 per extra node
+KERNEL_SFU_OPS = 4                # MUFU per point-eval in k_wilson<Sech2PackedF32> at Q = 1 (sqrt, rsqrt, 2 x ex2); + 2 per extra node;
+                                  # + 1/P: one reciprocal per staged point is shared by the P grid points of a thread
 
 
 def affinity_cores():
@@ -340,7 +341,8 @@ def run_ours(args, cfg):
             ops = ALG_PLAIN_OPS + ALG_SFU_OPS + (Q - 1) * (ALG_NODE_PLAIN_OPS + ALG_NODE_SFU_OPS)
             ops_how = ("%d algorithmic FP32 lane-ops per point-eval (29 plain + 7 special-function, SURVEY.md 8(d)%s)"
                        % (ops, "" if Q == 1 else "; + 21 + 4 per extra Gauss-Legendre node"))
-            pipe_frac = {"pipe": "xu", "ops_per_point_eval": KERNEL_SFU_OPS + 2 * (Q - 1),
+            P = 4 if (Q == 1 and cfg.n_T * cfg.n_rho >= 2048) else 2      # grid points per thread (launch_wilson_sech2_f32)
+            pipe_frac = {"pipe": "xu", "ops_per_point_eval": KERNEL_SFU_OPS + 2 * (Q - 1) + 1.0 / P,
                          "peak_lanes_per_clk_sm": SFU_LANES_PER_CLK_SM}
         else:
             ops = ALG_OPS_UNIFORM
