@@ -22,6 +22,7 @@
 //   laid out as NV4 float4 arrays followed by one float2 array (Q = 1 without phi_cm: exactly one LDS.128 + one LDS.64).
 #pragma once
 
+#include "wl_block_bounds.cuh"
 #include "wl_wilson_body.cuh"
 
 namespace wl {
@@ -222,49 +223,24 @@ struct Sech2PackedF32 : PackedF32Base<P_, THREADS_, HAS_PHI, Q_, MINB_> {
     }
     __device__ double b_scale() const { return 4.0 * eB0; }
 
-    // ---- far blocks --------------------------------------------------------------------------------------------
+    // ---- far blocks (wl_block_bounds.cuh) ------------------------------------------------------------------------
     // The near-axis polynomial, its select and the guard of rsqrt are needed only where a node can come within
-    // u^2 < 1/8 of the axis.  While staging, every warp records the bounding box of the 32 segments it stages
-    // (unit-loop coordinates); before a block of kSumBlock = 128 staged points is walked, every thread bounds
-    // rho_i^2(t) from below for its P grid points over the block's box, and if the whole WARP is clear of the axis
-    // the block runs an instantiation without those instructions.  The same bound limits E = 2^(-u') from above, and on
-    // a shorter range of E the polynomial for 1 - log2(1+E) reaches the same 6e-8 with a lower degree: kTiers
-    // instantiations of the walk, the tier being a function of the loop, the grid and the tile shape only.
+    // u^2 < 1/8 of the axis, and the bound that rules this out for a whole warp and block also limits E = 2^(-u') from
+    // above: on a shorter range of E the polynomial for 1 - log2(1+E) reaches the same 6e-8 with a lower degree.
+    // kTiers instantiations of the walk; tier 0 is the full code.
     static constexpr bool kBlockBounds = true;
-    static constexpr int kBoundsBlocks = B::kChunk / B::kSumBlock, kBoundsSlots = B::kSumBlock / 32;
-    static_assert(B::kSumBlock % 32 == 0 && B::kChunk % B::kSumBlock == 0, "a warp's 32 staged points lie in one block");
-    __host__ __device__ static constexpr size_t stage_bytes(int q) { return B::stage_bytes(q) + sizeof(float4) * kBoundsBlocks * kBoundsSlots; }
-
-    __device__ __forceinline__ static int ordered(float f) { const int i = __float_as_int(f); return i ^ ((i >> 31) & 0x7fffffff); }
-    __device__ __forceinline__ static float unordered(int i) { return __int_as_float(i ^ ((i >> 31) & 0x7fffffff)); }
-
-    // every thread of the CTA, once per staging step: ib = first staged index of the step, (y, z) = its segment
+    static constexpr int kBoundsBlock = B::kSumBlock;
+    typedef BlockBounds<B::kChunk, kBoundsBlock> Bounds;
+    __host__ __device__ static constexpr size_t stage_bytes(int q) { return B::stage_bytes(q) + Bounds::kBytes; }
     __device__ __forceinline__ void note_bounds(unsigned char* s, int ib, bool valid, double yx, double yy, double zx, double zy) const
     {
-        const float inf = __int_as_float(0x7f800000);
-        const float x0 = valid ? fminf(float(yx), float(zx)) : inf, x1 = valid ? fmaxf(float(yx), float(zx)) : -inf;
-        const float y0 = valid ? fminf(float(yy), float(zy)) : inf, y1 = valid ? fmaxf(float(yy), float(zy)) : -inf;
-        const float bx0 = unordered(__reduce_min_sync(0xffffffffu, ordered(x0))), bx1 = unordered(__reduce_max_sync(0xffffffffu, ordered(x1)));
-        const float by0 = unordered(__reduce_min_sync(0xffffffffu, ordered(y0))), by1 = unordered(__reduce_max_sync(0xffffffffu, ordered(y1)));
-        const int i0 = ib + (int)(threadIdx.x & ~31u);                 // first staged index of this warp's 32 points
-        if ((threadIdx.x & 31u) == 0 && i0 < B::kChunk)
-            reinterpret_cast<float4*>(s + B::stage_bytes(0))[i0 / 32] = make_float4(bx0, bx1, by0, by1);
+        Bounds::note(s + B::stage_bytes(0), ib, valid, yx, yy, zx, zy);
     }
-
-    // Tier of the block starting at staged index i0 = how far from the axis every node of the block stays for every grid
-    // point of this WARP: a lower bound of w' (conservative: the box bounds every point of every segment, the margins
-    // cover the FP32 rounding of w' and of this test) is compared with kTierW[].  Tier 0: the axis may be near.
     static constexpr int kTiers = 6;
     __device__ __forceinline__ static int block_tier(const unsigned char* s, int i0, const Grid& g)
     {
-        const float4* bb = reinterpret_cast<const float4*>(s + B::stage_bytes(0)) + (i0 / B::kSumBlock) * kBoundsSlots;
-        float4 b = bb[0];
-#pragma unroll
-        for (int k = 1; k < kBoundsSlots; ++k) {
-            const float4 c = bb[k];
-            b.x = fminf(b.x, c.x); b.y = fmaxf(b.y, c.y); b.z = fminf(b.z, c.z); b.w = fmaxf(b.w, c.w);
-        }
-        const float ext2 = fmaxf(b.x * b.x, b.y * b.y) + fmaxf(b.z * b.z, b.w * b.w);   // max |y|^2 over the box
+        const float4 b = Bounds::box(s + B::stage_bytes(0), i0);
+        const float ext2 = Bounds::extent2(b);
         float wlow = 1e30f;
 #pragma unroll
         for (int q = 0; q < NP; ++q) {
@@ -274,18 +250,9 @@ struct Sech2PackedF32 : PackedF32Base<P_, THREADS_, HAS_PHI, Q_, MINB_> {
             upk(g.Tt[q], Tt[0], Tt[1]);
             if (HAS_PHI) upk(g.ay[q], ay[0], ay[1]);
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                // k x_cm = (ax, ay)/(2 k sqrt T), k sqrt(T) = sqrt(Tt): the node is k x_cm + k sqrt(T) y, y in the box
-                const float t = xu_rsqrt(Tt[h]), ks = Tt[h] * t, cx = 0.5f * ax[h] * t, cy = 0.5f * ay[h] * t;
-                const float dx = fmaxf(fmaxf(fmaf(ks, b.x, cx), -fmaf(ks, b.y, cx)), 0.0f);
-                const float dy = fmaxf(fmaxf(fmaf(ks, b.z, cy), -fmaf(ks, b.w, cy)), 0.0f);
-                const float d2 = fmaf(dx, dx, dy * dy);
-                const float w = fmaf(d2, 0.999f, -1e-5f * fmaf(Tt[h], ext2, R2[h]));
-                wlow = (w >= 0.0f) ? fminf(wlow, w) : 0.0f;                   // a NaN counts as "near"
-            }
+            for (int h = 0; h < 2; ++h) wlow = fminf(wlow, Bounds::w_low(b, ext2, R2[h], ax[h], ay[h], Tt[h]));
         }
-        // non-negative floats order like their bit patterns
-        const float wwarp = __int_as_float(__reduce_min_sync(0xffffffffu, __float_as_int(wlow)));
+        const float wwarp = Bounds::warp_min(wlow);
         int tier = 0;
 #pragma unroll
         for (int k = 1; k < kTiers; ++k) tier = (wwarp >= tier_w(k)) ? k : tier;

@@ -22,7 +22,7 @@
 //   void stage(smem, i, yx, yy, zx, zy)                       derive and store point i (y) and its neighbour (z)
 //   void point(smem, i, grid, acc)                            add staged point i to the sums of all P grid points
 //   double g_scale(), b_scale()                               constant factors of phase and spin
-// Optional (a Term that declares kBlockBounds = true; needs kSumBlock > 0):
+// Optional (a Term that declares kBlockBounds = true; blocks of kSumBlock staged points, or of kBoundsBlock if kSumBlock = 0):
 //   void note_bounds(smem, ib, valid, yx, yy, zx, zy)         called by EVERY thread next to stage(): the Term keeps a
 //                                                             bounding box of every block of kSumBlock staged segments
 //   void block(smem, i0, ie, grid, acc)                       walks the block [i0, ie) itself instead of point() calls
@@ -292,6 +292,8 @@ __device__ __forceinline__ void wilson_body(const EvalArgs& a, const int n_grid,
                         }
                         acc.flush(grid, dph, dsp);
                     }
+                } else if constexpr (term_block_bounds<Term>::value) {
+                    for (int i0 = 0; i0 < cn; i0 += Term::kBoundsBlock) term.block(sStaged, i0, min(i0 + Term::kBoundsBlock, cn), grid, acc);
                 } else {
 #pragma unroll Term::kUnroll
                     for (int i = 0; i < cn; ++i) term.point(sStaged, i, grid, acc);
