@@ -45,9 +45,11 @@ ALG_NODE_SFU_OPS = 4
 ALG_OPS_UNIFORM = 4
 ALG_OPS_FLUXTUBE = 16             # 14 plain + 2 reciprocals
 # FP64 has no special-function unit: the seven elementary functions are counted as their shortest double-precision
-# sequences (2 x sqrt/rsqrt: 9, 2 x 2^x: 13, 2 x reciprocal: 4, log2(1+E): 20 -> 72) + the 29 plain ops.
-ALG_F64_OPS_SECH2 = 101
-KERNEL_F64_OPS_SECH2 = 97         # what k_wilson<Sech2LeanF64> issues on the FP64 pipe (one shared reciprocal)
+# sequences (2 x sqrt/rsqrt: 9, 2 x 2^x: 13, 2 x reciprocal: 4, log2(1+E): 3 -- the degree the polynomial needs far from
+# the axis, the easiest case; near it the same accuracy takes degree 20) + the 29 plain ops: 84.  Counting the easiest
+# case keeps `frac` a lower bound whatever mix of near and far blocks a workload has.
+ALG_F64_OPS_SECH2 = 84
+KERNEL_F64_OPS_SECH2 = 73         # FP64-pipe instructions k_wilson<Sech2LeanF64> issues per point-eval in its farthest tier (97 in tier 0)
 SM_COUNT = 148
 ISSUE_LANES_PER_CLK_SM = 128      # 4 sub-partitions x 1 warp instruction (32 lanes) per clock
 FP64_LANES_PER_CLK_SM = 64        # measured 63.8 (profiles/r01_pipe_rates.md)
@@ -355,8 +357,9 @@ def run_ours(args, cfg):
     else:
         if cfg.profile == 1:
             ops = ALG_F64_OPS_SECH2
-            ops_how = ("%d FP64 lane-ops per point-eval counted from the mathematics (29 plain + 72 for the seven "
-                       "elementary functions as shortest double-precision sequences, DESIGN.md section 5)" % ops)
+            ops_how = ("%d FP64 lane-ops per point-eval counted from the mathematics (29 plain + 55 for the seven "
+                       "elementary functions as shortest double-precision sequences, the logarithm at the degree it needs "
+                       "far from the axis; DESIGN.md section 5)" % ops)
             if Q == 1:
                 pipe_frac = {"pipe": "fp64", "ops_per_point_eval": KERNEL_F64_OPS_SECH2,
                              "peak_lanes_per_clk_sm": FP64_LANES_PER_CLK_SM}
@@ -369,7 +372,9 @@ def run_ours(args, cfg):
     if pipe_frac is not None:
         pipe_frac["frac"] = (pipe_frac["ops_per_point_eval"] * evals_per_gpu / (k_ms * 1e-3)) / (
             SM_COUNT * pipe_frac["peak_lanes_per_clk_sm"] * sm_max_mhz * 1e6)
-        pipe_frac["note"] = "instructions the kernel issues on its binding pipe (not an algorithmic count)"
+        pipe_frac["note"] = ("instructions the kernel issues on its binding pipe (not an algorithmic count)"
+                             + ("; the count of the farthest tier, tier 0 issues 97: a lower bound of the utilisation"
+                                if pipe_frac["pipe"] == "fp64" else ""))
     traffic, traffic_note = ncu_traffic(cfg.name, compute, args)
     roofline = {
         "bound": "alu", "kernel": "k_wilson", "achieved": achieved / 1e12, "peak": peak / 1e12,
