@@ -37,11 +37,14 @@ UNIT = "point-evals/s"
 
 # algorithmic work per point-eval of the sech^2 profile in FP32
 # (SURVEY.md section 8(d)): 29 plain FP32 lane-ops + 7 special-function lane-ops at the midpoint rule; every
-# further Gauss-Legendre node of eq. (24) adds one segment evaluation (21 plain + 4 special-function).
+# further Gauss-Legendre node of eq. (24) adds, in the easiest case (far from the axis, where the logarithm is a
+# degree-1 polynomial and the reciprocal is shared): radius 2, u' 1, 1+E 1, denominator product and its share of the
+# inverse 2, bracket 2, 1/w' 1, g 1, weighted sum 1 = 11 plain, and rsqrt + 2^x = 2 special-function lane-ops.
+# (The survey gives a count for the midpoint rule only; counting the easiest case keeps `frac` a lower bound.)
 ALG_PLAIN_OPS = 29
 ALG_SFU_OPS = 7
-ALG_NODE_PLAIN_OPS = 21
-ALG_NODE_SFU_OPS = 4
+ALG_NODE_PLAIN_OPS = 11
+ALG_NODE_SFU_OPS = 2
 ALG_OPS_UNIFORM = 4
 ALG_OPS_FLUXTUBE = 16             # 14 plain + 2 reciprocals
 # FP64 has no special-function unit: the seven elementary functions are counted as their shortest double-precision
@@ -342,7 +345,7 @@ def run_ours(args, cfg):
         if cfg.profile == 1:
             ops = ALG_PLAIN_OPS + ALG_SFU_OPS + (Q - 1) * (ALG_NODE_PLAIN_OPS + ALG_NODE_SFU_OPS)
             ops_how = ("%d algorithmic FP32 lane-ops per point-eval (29 plain + 7 special-function, SURVEY.md 8(d)%s)"
-                       % (ops, "" if Q == 1 else "; + 21 + 4 per extra Gauss-Legendre node"))
+                       % (ops, "" if Q == 1 else "; + 11 + 2 per extra Gauss-Legendre node"))
             P = 4 if (Q == 1 and cfg.n_T * cfg.n_rho >= 2048) else 2      # grid points per thread (launch_wilson_sech2_f32)
             pipe_frac = {"pipe": "xu", "ops_per_point_eval": KERNEL_SFU_OPS + 2 * (Q - 1) + 1.0 / P,
                          "peak_lanes_per_clk_sm": SFU_LANES_PER_CLK_SM}
