@@ -67,7 +67,7 @@ EvalArgs make_args(const wl_field* field, const void* d_loops, wl_dtype loop_dty
     a.T = d_T; a.rho = d_rho_cm; a.phi = d_phi_cm; a.n_T = n_T; a.n_rho = n_rho;
     a.p0 = field->p0; a.p1 = field->p1; a.scalar = field->scalar; a.disc = 0;
     a.quad = o.quad; a.seeded = o.seeded; a.bulk = o.bulk; a.seed = o.seed; a.loop_begin = o.loop_begin;
-    a.partial = nullptr; a.phase_out = nullptr; a.spin_out = nullptr;
+    a.partial = nullptr; a.partial_in_walk_order = 0; a.phase_out = nullptr; a.spin_out = nullptr;
     return a;
 }
 
@@ -226,13 +226,14 @@ wl_status wl_eval_opt(const wl_field* field, const void* d_loops, wl_dtype loop_
 
     EvalArgs a = make_args(field, d_loops, loop_dtype, n_loops, n_ppl, d_T, n_T, d_rho_cm, d_phi_cm, n_rho, o);
     a.partial = reinterpret_cast<double*>(d_workspace);
+    a.partial_in_walk_order = o.shuffle ? 0 : 1;          // shuffled groups: the array is W per loop, read as [t][r]
     cudaStream_t s = (cudaStream_t)stream;
     if (o.ev0 && cudaEventRecord((cudaEvent_t)o.ev0, s) != cudaSuccess) return launch_status(cudaErrorUnknown);
     cudaError_t e = launch_wilson(plan, a, field->profile, compute, s);
     if (e != cudaSuccess) return launch_status(e);
     if (o.ev1 && cudaEventRecord((cudaEvent_t)o.ev1, s) != cudaSuccess) return launch_status(cudaErrorUnknown);
     if (!o.shuffle)
-        return launch_status(launch_group_reduce(a.partial, plan.units_per_group, n_groups, plan.n_grid, n_loops,
+        return launch_status(launch_group_reduce(a.partial, plan.units_per_group, n_groups, n_T, n_rho, n_loops,
                                                  d_group_sums, d_W_mean, s));
     // shuffled groups: the workspace holds W per loop, then the membership table
     int32_t* perm = reinterpret_cast<int32_t*>(reinterpret_cast<unsigned char*>(d_workspace)
@@ -289,11 +290,12 @@ wl_status wl_eval_discretization(const wl_field* field, const void* d_loops, wl_
     EvalArgs a = make_args(field, d_loops, loop_dtype, n_loops, n_ppl, d_T, n_T, d_rho_cm, d_phi_cm, n_rho, Opt());
     a.disc = 1;
     a.partial = reinterpret_cast<double*>(d_workspace);
+    a.partial_in_walk_order = 1;
     cudaStream_t s = (cudaStream_t)stream;
     cudaError_t e = launch_wilson(plan, a, field->profile, compute, s);
     if (e != cudaSuccess) return launch_status(e);
     for (int lev = 0; lev < 3; ++lev) {
-        e = launch_group_reduce(a.partial + lev * level, plan.units_per_group, n_groups, plan.n_grid,
+        e = launch_group_reduce(a.partial + lev * level, plan.units_per_group, n_groups, n_T, n_rho,
                                 n_loops, d_group_sums3 + (size_t)lev * n_groups * plan.n_grid, nullptr, s);
         if (e != cudaSuccess) return launch_status(e);
     }

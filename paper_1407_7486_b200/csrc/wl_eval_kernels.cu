@@ -8,17 +8,21 @@ namespace wl {
 constexpr int kThreads = 256;
 
 // S_g = sum over the units of group g, in unit order (eq. (60)).  One thread per
-// (group, grid point); the group index is folded into blockIdx.x (any number of groups).
-__global__ void k_group_reduce(const double* __restrict__ partial, int64_t units_per_group, int n_grid,
+// (group, grid point); the group index is folded into blockIdx.x (any number of groups).  The partial sums come in
+// the order k_wilson walks the grid (coalesced on both sides); the group sums go out as [t][r].
+__global__ void k_group_reduce(const double* __restrict__ partial, int64_t units_per_group, int n_T, int n_rho,
                                int tiles, double* __restrict__ group_sums)
 {
-    const int k = (blockIdx.x % tiles) * blockDim.x + threadIdx.x;
+    const int n_grid = n_T * n_rho;
+    const int v = (blockIdx.x % tiles) * blockDim.x + threadIdx.x;
     const int64_t g = blockIdx.x / tiles;
-    if (k >= n_grid) return;
-    const double* p = partial + g * units_per_group * n_grid + k;
+    if (v >= n_grid) return;
+    const double* p = partial + g * units_per_group * n_grid + v;
     double S = 0.0;
     for (int64_t c = 0; c < units_per_group; ++c) S += p[c * n_grid];
-    group_sums[g * n_grid + k] = S;
+    int it, ir;
+    walk_position(v, n_T, n_rho, &it, &ir);
+    group_sums[g * n_grid + it * n_rho + ir] = S;
 }
 
 // <W> = (sum_g S_g)/N_l in group order (eq. (61)-(62)).
@@ -177,12 +181,13 @@ cudaError_t launch_wilson(const EvalPlan& plan, const EvalArgs& a, int profile, 
 }
 
 cudaError_t launch_group_reduce(const double* partial, int64_t units_per_group, int n_groups,
-                                int n_grid, int64_t n_loops, double* group_sums, double* W_mean,
+                                int n_T, int n_rho, int64_t n_loops, double* group_sums, double* W_mean,
                                 cudaStream_t s)
 {
+    const int n_grid = n_T * n_rho;
     const int tiles = (n_grid + 255) / 256;
     if ((int64_t)tiles * n_groups > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
-    k_group_reduce<<<(unsigned)(tiles * n_groups), 256, 0, s>>>(partial, units_per_group, n_grid, tiles, group_sums);
+    k_group_reduce<<<(unsigned)(tiles * n_groups), 256, 0, s>>>(partial, units_per_group, n_T, n_rho, tiles, group_sums);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     if (!W_mean) return cudaSuccess;

@@ -157,11 +157,12 @@ extern "C" wl_status wl_eval_host(const wl_field* field, const void* h_loops, wl
         a.p0 = field->p0; a.p1 = field->p1; a.scalar = field->scalar; a.disc = 0;
         a.quad = 1; a.seeded = 0; a.bulk = 0; a.seed = 0; a.loop_begin = 0;
         a.partial = partial + (size_t)(l0 / plan.loops_per_unit) * plan.n_grid;
+        a.partial_in_walk_order = 1;
         a.phase_out = nullptr; a.spin_out = nullptr;
         cudaError_t e = wl::launch_wilson(sub, a, field->profile, compute, d.s);
         if (e != cudaSuccess) { cudaGetLastError(); return e == cudaErrorInvalidValue ? WL_ERR_UNSUPPORTED : WL_ERR_CUDA; }
     }
-    if (wl::launch_group_reduce(partial, plan.units_per_group, n_groups, plan.n_grid, n_loops,
+    if (wl::launch_group_reduce(partial, plan.units_per_group, n_groups, n_T, n_rho, n_loops,
                                 reinterpret_cast<double*>(d.p[GS]), mean, d.s) != cudaSuccess) {
         cudaGetLastError();
         return WL_ERR_CUDA;

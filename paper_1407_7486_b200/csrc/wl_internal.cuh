@@ -34,6 +34,17 @@ struct EvalPlan {
 EvalPlan make_eval_plan(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups, wl_dtype compute,
                         bool per_loop, int64_t ensemble_loops = 0);
 
+// The order in which k_wilson walks the (T, rho_cm) grid (wl_wilson_body.cuh): strips of kRhoStrip neighbouring
+// rho_cm, within a strip rho_cm fastest, then the proper time; the last strip may be narrower.  Position v of the walk
+// is grid point (*it, *ir).
+constexpr int kRhoStrip = 8;
+__host__ __device__ inline void walk_position(int v, int n_T, int n_rho, int* it, int* ir)
+{
+    const int nb = n_rho / kRhoStrip, rem = n_rho % kRhoStrip, full = nb * kRhoStrip * n_T;
+    if (v < full) { const int blk = v / (kRhoStrip * n_T), w = v % (kRhoStrip * n_T); *it = w / kRhoStrip; *ir = blk * kRhoStrip + w % kRhoStrip; }
+    else { const int w = v - full; *it = w / rem; *ir = nb * kRhoStrip + w % rem; }
+}
+
 struct EvalArgs {
     const void* loops;          // [n_loops][n_ppl][2]; unused when seeded
     int loops_are_f64;          // storage precision of the loop coordinates (also the rounding a seeded run emulates)
@@ -52,6 +63,8 @@ struct EvalArgs {
     uint64_t seed;
     int64_t loop_begin;
     double* partial;            // [n_units][n_grid]
+    int partial_in_walk_order;  // 1: partial[unit][v], v = position in the grid walk (coalesced; k_group_reduce maps it back);
+                                // 0: partial[unit][t * n_rho + r] (per-loop and shuffled paths: the array is an output)
     double* phase_out;          // per-loop mode only, nullable
     double* spin_out;           // per-loop mode only, nullable
 };
@@ -67,8 +80,9 @@ cudaError_t launch_wilson_sech2_f64(const EvalPlan& plan, const EvalArgs& a, cud
 // Is (quadrature order, phi_cm, discretisation, staging) a combination the lean kernels are instantiated for?
 bool lean_combination(const EvalArgs& a);
 
+// partial is [n_units][n_grid] in WALK order (EvalArgs::partial_in_walk_order = 1); group_sums and W_mean are [t][r]
 cudaError_t launch_group_reduce(const double* partial, int64_t units_per_group, int n_groups,
-                                int n_grid, int64_t n_loops, double* group_sums, double* W_mean,
+                                int n_T, int n_rho, int64_t n_loops, double* group_sums, double* W_mean,
                                 cudaStream_t s);
 cudaError_t launch_group_permutation(uint64_t seed, int64_t n_loops, int n_T, int32_t* perm, cudaStream_t s);
 cudaError_t launch_group_reduce_shuffled(const double* W_loop, const int32_t* perm, int64_t n_loops, int n_T,

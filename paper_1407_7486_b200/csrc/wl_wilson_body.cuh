@@ -97,8 +97,6 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
 template <class T, class = void> struct term_block_bounds { static constexpr bool value = false; };
 template <class T> struct term_block_bounds<T, decltype((void)T::kBlockBounds)> { static constexpr bool value = T::kBlockBounds; };
 
-constexpr int kRhoStrip = 8;     // width in rho_cm of the strips the grid is walked in (wilson_body)
-
 // Shared memory a launch needs beyond the staged chunk.
 template <class Term>
 __host__ __device__ inline size_t wilson_extra_smem(int n_ppl, bool seeded, bool bulk, bool loops_are_f64)
@@ -135,7 +133,7 @@ __device__ __forceinline__ void wilson_body(const EvalArgs& a, const int n_grid,
     // about one distance at about one loop size, which is what lets a Term choose one code path for all of its lanes
     // (wl_terms_packed_f32.cuh, "far blocks").  gp[j] = t * n_rho + r is the point's index in every output array.
     typename Term::Grid grid;
-    int gp[P];
+    int gp[P], vp[P];                                     // output index and walk position
     unsigned gp_ok = 0;
     {
         double Tj[P], rj[P], cxj[P], cyj[P];
@@ -144,11 +142,9 @@ __device__ __forceinline__ void wilson_body(const EvalArgs& a, const int n_grid,
             const int v = ((tile * (THREADS / 32) + (tid >> 5)) * P + j) * 32 + (tid & 31);
             if (v < n_grid) gp_ok |= 1u << j;
             const int vc = min(v, n_grid - 1);
-            constexpr int RB = kRhoStrip;
-            const int nb = a.n_rho / RB, rem = a.n_rho % RB, full = nb * RB * a.n_T;
             int it, ir;
-            if (vc < full) { const int blk = vc / (RB * a.n_T), w = vc % (RB * a.n_T); it = w / RB; ir = blk * RB + w % RB; }
-            else { const int w = vc - full; it = w / rem; ir = nb * RB + w % rem; }
+            walk_position(vc, a.n_T, a.n_rho, &it, &ir);
+            vp[j] = vc;
             gp[j] = it * a.n_rho + ir;
             Tj[j] = a.T[it];
             rj[j] = a.rho[ir];
@@ -330,7 +326,7 @@ __device__ __forceinline__ void wilson_body(const EvalArgs& a, const int n_grid,
     for (int v = 0; v < kLevels; ++v)
 #pragma unroll
         for (int j = 0; j < P; ++j)
-            if (gp_ok >> j & 1) a.partial[((int64_t)v * n_units + unit) * n_grid + gp[j]] = Wsum[v][j];
+            if (gp_ok >> j & 1) a.partial[((int64_t)v * n_units + unit) * n_grid + (a.partial_in_walk_order ? vp[j] : gp[j])] = Wsum[v][j];
 }
 
 template <class Term, bool DISC, bool BULK>
