@@ -84,6 +84,27 @@ def test_every_tier_against_the_oracle(api, o, n_T, n_rho, lam, compute):
 
 
 @pytest.mark.parametrize("compute", ["f32", "f64"])
+@pytest.mark.parametrize("n_T,n_rho", [(16, 128), (6, 24)])
+def test_every_tier_with_phi_cm(api, o, n_T, n_rho, compute):
+    """The same with the centres of mass spread round the axis (phi_cm given: the HAS_PHI Terms, whose bound uses both
+    components of x_cm); smooth loops are not isotropic, so a wrong sign or a swapped component in the bound would put
+    near blocks into a far tier for some angles."""
+    n_loops, N, lam = 5, 1024, 0.5
+    y = smooth_loops(n_loops, N, 23 + n_rho, 0.6 * lam)
+    T = np.geomspace(0.0025, 9.0, n_T)
+    rho = lam * np.concatenate([[0.0, 0.2, 0.45], np.geomspace(0.6, 25.0, n_rho - 3)])
+    phi = 2.0 * np.pi * ((np.arange(n_rho) * 0.381966) % 1.0)         # golden-angle spread
+    params = (1.7 / lam ** 2, lam)
+    f = api.wl_field_create(SECH2, params)
+    loops = torch.tensor(y, dtype=torch.float32 if compute == "f32" else torch.float64, device="cuda")
+    ref = o.evaluate(SECH2, params, loops.cpu().numpy().astype(np.float64), T, rho, phi, per_loop=True)
+    W, p, s = api.wl_eval_per_loop(f, loops, dev(T), dev(rho), dev(phi), compute=compute)
+    torch.cuda.synchronize()
+    per_loop_close((W.cpu().numpy(), p.cpu().numpy(), s.cpu().numpy()), ref, "phi_cm n_T=%d n_rho=%d" % (n_T, n_rho), compute)
+    assert np.abs(ref["phase"]).max() > 0.5
+
+
+@pytest.mark.parametrize("compute", ["f32", "f64"])
 def test_a_block_that_crosses_the_axis_inside_a_far_warp(api, o, compute):
     """One grid point sits exactly where the loop passes (its nodes reach w' ~ 0), the other 127 of its warp are far
     away: the warp must take tier 0 for that block, and the far lanes must not notice."""
