@@ -1,21 +1,22 @@
 // wl_terms_packed_f32.cuh -- the packed-FP32 Terms of k_wilson (wl_wilson_body.cuh): Sech2PackedF32 (the kernel
 // configs 3, 4 and 5 of BASELINE.json are timed on) and FluxTubePackedF32 (the paper's validation profile,
 // eq. (68)).  CUDA path, sm_100a only.  The per-term arithmetic is arranged for the two resources that bound
-// it on B200 (profiles/r01_pipe_rates.md):
+// it on B200 (profiles/r01_pipe_rates.md, profiles/r02_variants.md):
 //
-//   * the special-function (XU) pipe, 16 lanes/clk/SM: one warp instruction per 8 clk per
-//     sub-partition, and each MUFU also costs two issue slots;
-//   * the issue slots, 1 warp instruction/clk/sub-partition.
+//   * the special-function (XU) pipe, 16 lanes/clk/SM: one warp instruction per 8 clk per sub-partition;
+//   * the FMA pipe: one packed FFMA2 per 2 clk per sub-partition, and next to a stream of FMA-pipe work every MUFU
+//     also takes 2-3 of that pipe's issue cycles.
 //
 // So (i) the plain FP32 work is issued as PACKED fma/mul/add.f32x2 (FFMA2: two grid points per
 // instruction, one issue slot), every thread owning P grid points as P/2 register pairs; (ii) the
 // staged loop values enter FFMA2 as both-halves scalar operands, so a staged point costs one LDS.128 and
 // one LDS.64 (shared-memory loads return through the same queue as the special-function results: every
 // 4 bytes per lane cost about one XU-pipe clock, profiles/r01_pipe_rates.md); (iii) the special-function
-// count per point-eval of the sech^2 profile is 3 + 2Q (Q = Gauss-Legendre points of eq. (24); 5 at Q = 1):
+// count per point-eval of the sech^2 profile is 2 + 2Q + 1/P (Q = Gauss-Legendre points of eq. (24); 4.25 at Q = 1, P = 4):
 //       sqrt(|x_i|^2), 2^(-u_p), [rsqrt(rho_i^2(t_q)), 2^(-u_q)] x Q, and ONE reciprocal per staged point and THREAD
-//   (the product of the denominators (1+E_p) prod_q (1+E_q) of all P grid points is inverted once), i.e. 2 + 2Q + 1/P;
-//   log2(1+E_q) is a degree-8 polynomial in E_q in [0,1] on the FMA pipe.
+//   (the product of the denominators (1+E_p) prod_q (1+E_q) of all P grid points is inverted once);
+//   log2(1+E_q) is a polynomial in E_q on the FMA pipe (degree 8 on [0,1], lower in the far-block tiers);
+//   (iv) blocks of staged points that stay clear of the axis for a whole warp run shorter code (far blocks, below).
 //
 // Staged record of a point i (floats; C = 2 values per position without phi_cm, 3 with):
 //     [ y_x, (y_y), |y|^2 ]  [ y(t_q)_x, (y(t_q)_y), |y(t_q)|^2 ] x Q  [ dy_y/2, (dy_x/2), y_i x y_{i+1} ]
@@ -195,7 +196,7 @@ struct PackedF32Base {
 // (coefficients: gen_h_poly.py hs 0.125 3, relative error 8e-8).
 // ------------------------------------------------------------------------------------------------------------
 // SCALAR_ = true (scalar QED, W = cos(phase)): the spin sum is not needed, so the point's
-// sqrt and 2^x are skipped and the reciprocal is that of the nodes alone: 3 MUFU per point-eval at Q = 1.
+// sqrt and 2^x are skipped and the reciprocal is that of the nodes alone: 2 + 1/P MUFU per point-eval at Q = 1.
 template <int P_, int THREADS_, bool HAS_PHI, int Q_, int MINB_ = 4, bool SCALAR_ = false>
 struct Sech2PackedF32 : PackedF32Base<P_, THREADS_, HAS_PHI, Q_, MINB_> {
     static_assert(!SCALAR_ || Q_ == 1, "the scalar-only variant is compiled for the midpoint rule");

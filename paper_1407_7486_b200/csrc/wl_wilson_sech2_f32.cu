@@ -24,7 +24,7 @@ cudaError_t launch_shape(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s
     if (a.quad == 1) {
         if (phi) return launch_term<Sech2PackedF32<P, TH, true, 1>, false, false>(plan, a, s);
         if (P == 4 && bulk_ok(a)) return launch_term<Sech2PackedF32<4, 256, false, 1>, false, true>(plan, a, s);
-        // scalar loops (W = cos(phase)) in the reducing path: the spin sum is not computed (3 MUFU per point-eval);
+        // scalar loops (W = cos(phase)) in the reducing path: the spin sum is not computed (2 + 1/P MUFU per point-eval);
         // the per-loop triage path keeps the full kernel so that its spin output stays meaningful
         if (a.scalar && !a.phase_out && !a.spin_out) return launch_term<Sech2PackedF32<P, TH, false, 1, 4, true>, false, false>(plan, a, s);
         return launch_term<Sech2PackedF32<P, TH, false, 1>, false, false>(plan, a, s);
