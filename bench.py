@@ -419,15 +419,24 @@ def run_ours(args, cfg):
     return 0
 
 
+def _code_only(text):
+    """C/C++ source without comments and with white space collapsed (string literals in the kernels hold no comment marks)."""
+    import re
+    text = re.sub(r"/\*.*?\*/", " ", text, flags=re.S)
+    text = re.sub(r"//[^\n]*", " ", text)
+    return " ".join(text.split())
+
+
 def source_sha16():
-    """sha256 (first 16 hex digits) of the kernel sources: ties an ncu capture to the code that was profiled."""
+    """sha256 (first 16 hex digits) of the kernel sources, comments and white space left out: ties an ncu capture to the
+    CODE that was profiled (editing a comment does not orphan a capture)."""
     import hashlib
     h = hashlib.sha256()
     csrc = os.path.join(ROOT, "paper_1407_7486_b200", "csrc")
     files = sorted(f for f in os.listdir(csrc) if f.endswith((".cu", ".cuh"))) if os.path.isdir(csrc) else []
     for f in files:
-        with open(os.path.join(csrc, f), "rb") as fh:
-            h.update(f.encode() + b"\0" + fh.read())
+        with open(os.path.join(csrc, f), "r", encoding="utf-8", errors="replace") as fh:
+            h.update(f.encode() + b"\0" + _code_only(fh.read()).encode())
     return h.hexdigest()[:16]
 
 
