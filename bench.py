@@ -57,9 +57,9 @@ SM_COUNT = 148
 ISSUE_LANES_PER_CLK_SM = 128      # 4 sub-partitions x 1 warp instruction (32 lanes) per clock
 FP64_LANES_PER_CLK_SM = 64        # measured 63.8 (profiles/r01_pipe_rates.md)
 SFU_LANES_PER_CLK_SM = 16         # measured 15.9
-KERNEL_SFU_OPS = 4                # MUFU per point-eval in k_wilson<Sech2PackedF32> at Q = 1 (sqrt, rsqrt, 2 x ex2); + 2 per extra node;
-                                  # + 1/P: one reciprocal per staged point is shared by the P grid points of a thread
-
+KERNEL_SFU_OPS = 4                # MUFU per point-eval in k_wilson<Sech2PackedF32> at Q = 1 (sqrt, rsqrt, 2 x ex2); + 2 per extra node.
+                                  # The one reciprocal per staged point and thread runs on the FMA pipe (256-thread kernels
+                                  # without phi_cm) or is a MUFU shared by the P = 2 grid points of a thread (grids <= 256 points)
 
 def affinity_cores():
     try:
@@ -346,8 +346,8 @@ def run_ours(args, cfg):
             ops = ALG_PLAIN_OPS + ALG_SFU_OPS + (Q - 1) * (ALG_NODE_PLAIN_OPS + ALG_NODE_SFU_OPS)
             ops_how = ("%d algorithmic FP32 lane-ops per point-eval (29 plain + 7 special-function, SURVEY.md 8(d)%s)"
                        % (ops, "" if Q == 1 else "; + 11 + 2 per extra Gauss-Legendre node"))
-            P = 4 if (Q == 1 and cfg.n_T * cfg.n_rho >= 2048) else 2      # grid points per thread (launch_wilson_sech2_f32)
-            pipe_frac = {"pipe": "xu", "ops_per_point_eval": KERNEL_SFU_OPS + 2 * (Q - 1) + 1.0 / P,
+            small = cfg.n_T * cfg.n_rho <= 256 or cfg.circle_radius is not None   # 128-thread or phi_cm kernel: MUFU reciprocal
+            pipe_frac = {"pipe": "xu", "ops_per_point_eval": KERNEL_SFU_OPS + 2 * (Q - 1) + (0.5 if small else 0.0),
                          "peak_lanes_per_clk_sm": SFU_LANES_PER_CLK_SM}
         else:
             ops = ALG_OPS_UNIFORM

@@ -279,9 +279,12 @@ struct Sech2PackedF32 : PackedF32Base<P_, THREADS_, HAS_PHI, Q_, MINB_> {
     // 1/t for a positive, normal t on the FMA pipe: the integer seed 0x7EF311C7 - bits(t) is within 12.6 %, three Newton
     // steps r <- r (2 - t r) bring that to 6e-8 (the accuracy of MUFU.RCP).  Six scalar FMA-pipe instructions and one
     // integer subtraction per thread and staged point instead of a special-function op: the XU pipe is the kernel's bound.
-    // (measured: 139.7 -> 135.4 ms on config 3; the scalar-only variant, 2.25 special-function ops per point-eval, is
-    // FMA-pipe bound and keeps the MUFU: 83.0 against 87.8 ms)
-    static constexpr bool kFmaRcp = !SCALAR_;
+    // (measured: 139.7 -> 135.4 ms on config 3.  Kept on the MUFU where the FMA pipe or latency binds instead: the
+    // scalar-only variant with its 2.25 special-function ops per point-eval (83.0 against 87.8 ms), the phi_cm variant with
+    // its third component per radius and phase sum (41.9 against 42.7 ms on 4096 loops), and the 128-thread variant of
+    // grids of at most 256 points, whose launches are too short to hide the longer dependent chain (config 1: 0.099
+    // against 0.104 ms).)
+    static constexpr bool kFmaRcp = !SCALAR_ && !HAS_PHI && THREADS_ >= 256;
     __device__ __forceinline__ static float fma_rcp(float t)
     {
         float r = __int_as_float(0x7EF311C7 - __float_as_int(t));
