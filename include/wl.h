@@ -49,7 +49,9 @@ typedef enum {
     WL_ERR_INVALID_ARG = 1,   /* null pointer, bad size, bad parameter value     */
     WL_ERR_UNSUPPORTED = 2,   /* valid request this build has no kernel for      */
     WL_ERR_WORKSPACE = 3,     /* workspace null or smaller than *_workspace_bytes */
-    WL_ERR_CUDA = 4           /* a CUDA runtime call failed (no device, launch)  */
+    WL_ERR_CUDA = 4,          /* a CUDA runtime call failed (no device, launch)  */
+    WL_ERR_STATIC_LIMIT = 5   /* wl_eval_static only: the sizes need more scratch than the library's
+                                 built-in array holds (wl_eval_static_max_bytes); use wl_eval */
 } wl_status;
 
 /* Field profiles B_z(rho), gauge A = A_phi(rho) e_phi, A_phi = Phi(rho)/(2 pi rho)
@@ -125,6 +127,37 @@ wl_status wl_eval(const wl_field* field,
                   int n_groups, wl_dtype compute,
                   double* d_W_mean, double* d_group_sums,
                   void* d_workspace, size_t workspace_bytes, void* stream);
+
+/* wl_eval for a caller that cannot allocate device memory and has no buffer to lend as workspace.
+ *
+ * wl_eval keeps its per-unit partial sums (k_wilson writes them, the group reduction of eq. (60),
+ * PAPER.md:386, 399, reads them) in a workspace the caller allocates.  Some callers cannot: a program
+ * that gave all of HBM to its own pool when it started, so that a cudaMalloc now fails; a plug-in or
+ * callback running where its host application forbids cudaMalloc / cudaFree because both stall every
+ * stream of the device; a job whose device-memory budget was fixed before launch.  For them the same
+ * evaluation runs with the partial sums in an array that is part of the library's device image:
+ *   - the array is wl_eval_static_max_bytes() = 16 MiB, present on every GPU that has used this entry
+ *     point (or whose CUDA module holding it was loaded) until the process exits, used or not;
+ *   - sizes with wl_eval_workspace_bytes(...) above that limit are refused with WL_ERR_STATIC_LIMIT
+ *     before anything is enqueued (BASELINE.json's config 1 needs 2 MiB; the paper-scale ones do not fit);
+ *   - the call makes no cudaMalloc, cudaFree or other allocating call, on the host or on the device; the
+ *     caller passes inputs and outputs exactly as to wl_eval, and the results have wl_eval's bits;
+ *   - the first call on each device looks the array's address up (cudaGetSymbolAddress, with that device
+ *     current, which may load the module) and caches it: make that first call during set-up, on the
+ *     device the later calls will use, and before any stream capture is begun;
+ *   - there is ONE array per device and every call uses it, keeping whatever the last call left there.
+ *     No clearing is needed (each call writes every partial sum before reading it), but two calls whose
+ *     kernels can overlap on the GPU -- different streams, or different host threads on different
+ *     streams -- race on it and both results are garbage.  Calls on one stream are ordered and safe.
+ * Plain midpoint rule, stored loops, contiguous groups only (no options block).
+ * Errors: as wl_eval; WL_ERR_STATIC_LIMIT as above; WL_ERR_CUDA if the address look-up fails. */
+size_t wl_eval_static_max_bytes(void);
+wl_status wl_eval_static(const wl_field* field,
+                         const void* d_loops, wl_dtype loop_dtype, int64_t n_loops, int n_ppl,
+                         const double* d_T, int n_T,
+                         const double* d_rho_cm, const double* d_phi_cm, int n_rho,
+                         int n_groups, wl_dtype compute,
+                         double* d_W_mean, double* d_group_sums, void* stream);
 
 /* Host helper: WL_OK if every h_T[k] is finite and > 0 and every h_rho_cm[k] is finite and >= 0
  * ("T <= 0, negative rho_cm -> invalid"), else WL_ERR_INVALID_ARG.

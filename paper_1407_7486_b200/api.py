@@ -49,6 +49,10 @@ _lib.wl_eval_launch_count.argtypes = [_i64, _int, _int, _int, _int, _int]
 _lib.wl_eval.restype = _int
 _lib.wl_eval.argtypes = [_vp, _vp, _int, _i64, _int, _dp, _int, _dp, _dp, _int, _int, _int, _dp, _dp,
                          _vp, _sz, _vp]
+_lib.wl_eval_static.restype = _int
+_lib.wl_eval_static.argtypes = list(_lib.wl_eval.argtypes[:14]) + [_vp]
+_lib.wl_eval_static_max_bytes.restype = _sz
+_lib.wl_eval_static_max_bytes.argtypes = []
 _lib.wl_eval_instrumented.restype = _int
 _lib.wl_eval_instrumented.argtypes = list(_lib.wl_eval.argtypes) + [_vp, _vp]
 
@@ -284,6 +288,34 @@ def wl_eval(field, loops, T, rho_cm, phi_cm=None, n_groups=1, compute=torch.floa
         else:
             e0, e1 = (_event_handle(ev, stream) for ev in wilson_events)
             _check(_lib.wl_eval_instrumented(*args, _stream(stream), e0, e1), "wl_eval_instrumented")
+    return W_mean, group_sums
+
+
+def wl_eval_static_max_bytes() -> int:
+    """Size of the library's built-in scratch array, the ceiling of wl_eval_static (bytes)."""
+    return int(_lib.wl_eval_static_max_bytes())
+
+
+def wl_eval_static(field, loops, T, rho_cm, phi_cm, n_groups, compute, W_mean, group_sums, stream=None):
+    """wl_eval for callers that may not allocate device memory (include/wl.h, wl_eval_static).
+
+    Nothing is allocated here either, in the library or in this binding: W_mean [n_T][n_rho] and group_sums
+    [G][n_T][n_rho] must be float64 CUDA tensors the caller already owns, and the partial sums go to a 16 MiB
+    array built into libwl.so (sizes that need more raise WLError with status WL_ERR_STATIC_LIMIT = 5).
+    That array is shared by every call on the device: keep calls on one stream, or otherwise ordered."""
+    n_loops, n_ppl = _loops_arg(loops)
+    T = _cuda_f64(T, "T")
+    rho_cm = _cuda_f64(rho_cm, "rho_cm")
+    n_T, n_rho = T.numel(), rho_cm.numel()
+    phi_cm = _cuda_f64(phi_cm, "phi_cm", n_rho)
+    if W_mean is None or group_sums is None:
+        raise ValueError("wl_eval_static allocates nothing: pass W_mean and group_sums")
+    _cuda_f64(W_mean, "W_mean", n_T * n_rho)
+    _cuda_f64(group_sums, "group_sums", n_groups * n_T * n_rho)
+    with torch.cuda.device(loops.device):
+        _check(_lib.wl_eval_static(field._h, _ptr(loops), _dtype_code(loops.dtype), n_loops, n_ppl, _ptr(T), n_T,
+                                   _ptr(rho_cm), _ptr(phi_cm), n_rho, int(n_groups), _dtype_code(compute),
+                                   _ptr(W_mean), _ptr(group_sums), _stream(stream)), "wl_eval_static")
     return W_mean, group_sums
 
 

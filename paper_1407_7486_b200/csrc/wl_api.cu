@@ -353,6 +353,7 @@ const char* wl_status_string(wl_status status)
         case WL_ERR_UNSUPPORTED: return "unsupported configuration";
         case WL_ERR_WORKSPACE: return "workspace missing or too small";
         case WL_ERR_CUDA: return "CUDA runtime error";
+        case WL_ERR_STATIC_LIMIT: return "sizes need more scratch than wl_eval_static's built-in array (wl_eval_static_max_bytes): use wl_eval with a workspace";
     }
     return "unknown status";
 }
