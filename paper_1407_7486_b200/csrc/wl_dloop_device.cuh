@@ -24,7 +24,7 @@
 
 namespace wl {
 
-constexpr int kSkeletonMax = 128;      // skeleton points per loop: N / Cg <= 128
+constexpr int kSkeletonMax = 256;      // skeleton points per loop: N / Cg <= 65536 / 256 (the shortest chunk any Term stages)
 constexpr int kClasses = 256;          // residue classes of the centre-of-mass sum
 
 // Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11), from the published description: ten

@@ -16,7 +16,7 @@ struct wl_field {
 
 namespace wl {
 
-constexpr int kMaxPplSeeded = 1 << 16;   // generator / seeded-evaluation limit on N (skeleton of <= 128 points)
+constexpr int kMaxPplSeeded = 1 << 16;   // generator / seeded-evaluation limit on N (skeleton of <= kSkeletonMax points, wl_dloop_device.cuh)
 
 // ---- how wl_eval cuts the work (a function of the sizes only, never of the device) ----
 struct EvalPlan {

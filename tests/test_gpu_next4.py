@@ -56,6 +56,7 @@ def grids(n_T, n_rho, T_max=6.0, rho_max=3.0, phi=False):
     (SECH2, (1.0, 1.0), "f32", "f32", 4, 65536, 8, 40, 2, False),       # the longest loop: skeleton of 64 points
     (SECH2, (1.0, 1.0), "f64", "f64", 2, 65536, 4, 40, 2, False),       # ... of 128 points (chunks of 512)
     (FLUX, (10.0, 1.0), "f64", "f32", 4, 16384, 4, 40, 2, False),       # generic FP64 kernel: chunks of 256, skeleton of 64
+    (FLUX, (10.0, 1.0), "f64", "f64", 2, 65536, 3, 40, 2, False),       # ... the longest loop there: skeleton of 256 points
 ])
 def test_seeded_equals_generate_then_eval_bit_for_bit(api, profile, params, compute, storage, n_loops, N, nT, nr, G, phi):
     T, rho, ph = grids(nT, nr, phi=phi)
