@@ -1,7 +1,7 @@
 // wl_terms_packed_f32.cuh -- the packed-FP32 Terms of k_wilson (wl_wilson_body.cuh): Sech2PackedF32 (the kernel
 // configs 3, 4 and 5 of BASELINE.json are timed on) and FluxTubePackedF32 (the paper's validation profile,
 // eq. (68)).  CUDA path, sm_100a only.  The per-term arithmetic is arranged for the two resources that bound
-// it on B200 (profiles/r01_pipe_rates.md, profiles/r02_variants.md):
+// it on B200 (profiles/r01_pipe_rates.md, profiles/r03_wilson_f32_ncu.md, "Tried"):
 //
 //   * the special-function (XU) pipe, 16 lanes/clk/SM: one warp instruction per 8 clk per sub-partition;
 //   * the FMA pipe: one packed FFMA2 per 2 clk per sub-partition, and next to a stream of FMA-pipe work every MUFU

@@ -66,7 +66,7 @@ __device__ __forceinline__ void segment_node(double yx, double yy, double zx, do
     n2 = nx * nx + ny * ny;
 }
 
-// ---- cp.async.bulk + mbarrier (the staging variant north_star names; measured in profiles/r02_staging.md) ----
+// ---- cp.async.bulk + mbarrier (the staging variant north_star names; measured in profiles/r03_wilson_f32_ncu.md, "Tried") ----
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
 {
@@ -101,6 +101,8 @@ template <class T> struct term_block_bounds<T, decltype((void)T::kBlockBounds)> 
 template <class Term>
 __host__ __device__ inline size_t wilson_extra_smem(int n_ppl, bool seeded, bool bulk, bool loops_are_f64)
 {
+    // every seeded loop the ABI accepts must fit the skeleton array: a shorter chunk than this would overrun it silently
+    static_assert(kMaxPplSeeded / Term::kChunk <= kSkeletonMax, "DLoopScratch::skel is too small for this Term's chunk length");
     size_t b = 0;
     if (seeded) {
         const DLoopShape sh = dloop_shape(n_ppl, Term::kChunk);
@@ -110,7 +112,9 @@ __host__ __device__ inline size_t wilson_extra_smem(int n_ppl, bool seeded, bool
     return b;
 }
 
-template <class Term, bool DISC, bool BULK>
+// SEEDED is a template parameter (like DISC and BULK) so that the stored-loop kernels -- the ones the benchmarks
+// time -- do not carry the FP64 Philox / Box-Muller generator in their code and register allocation.
+template <class Term, bool DISC, bool BULK, bool SEEDED>
 __device__ __forceinline__ void wilson_body(const EvalArgs& a, const int n_grid, const int n_tiles,
                                             const int loops_per_unit, const int64_t n_units)
 {
@@ -163,7 +167,8 @@ __device__ __forceinline__ void wilson_body(const EvalArgs& a, const int n_grid,
         for (int j = 0; j < P; ++j) Wsum[v][j] = 0.0;
 
     // ---- seeded mode: the loop is regenerated chunk by chunk in shared memory (wl_dloop_device.cuh) ----
-    const bool seeded = !DISC && !BULK && a.seeded;
+    static_assert(!SEEDED || (!DISC && !BULK), "seeded evaluation: ordinary pass, ordinary staging only");
+    constexpr bool seeded = SEEDED;
     DLoopShape shp = dloop_shape(N, CHUNK);
     double2* const yraw = reinterpret_cast<double2*>(sExtra);
     DLoopScratch* const sc = reinterpret_cast<DLoopScratch*>(sExtra + sizeof(double2) * (size_t)(shp.Cg + 1));
@@ -200,7 +205,7 @@ __device__ __forceinline__ void wilson_body(const EvalArgs& a, const int n_grid,
         const int64_t loop = unit * loops_per_unit + ll;
         const double2* L64 = reinterpret_cast<const double2*>(a.loops) + loop * N;
         const float2* L32 = reinterpret_cast<const float2*>(a.loops) + loop * N;
-        if (seeded) {
+        if constexpr (seeded) {
             __syncthreads();                                  // the previous loop's last chunk has been consumed
             dloop_begin(a.seed, (uint64_t)(a.loop_begin + loop), shp, sc, yraw);
         }
@@ -229,7 +234,7 @@ __device__ __forceinline__ void wilson_body(const EvalArgs& a, const int n_grid,
             for (int c0 = 0; c0 < Nv; c0 += CHUNK) {
                 const int cn = min(CHUNK, Nv - c0);
                 __syncthreads();                              // the previous chunk has been consumed
-                if (seeded) dloop_chunk(a.seed, (uint64_t)(a.loop_begin + loop), shp, c0 / CHUNK, sc->skel, yraw);
+                if constexpr (seeded) dloop_chunk(a.seed, (uint64_t)(a.loop_begin + loop), shp, c0 / CHUNK, sc->skel, yraw);
                 const unsigned char* ring = sRing + (size_t)(ring_idx & 1) * (CHUNK + 2) * raw_elem;
                 if (BULK) mbar_wait(sBar + (ring_idx & 1), (uint32_t)((ring_idx >> 1) & 1));
                 for (int ib = 0; ib < cn; ib += THREADS) {    // stage: derived unit-loop quantities, FP64
@@ -245,7 +250,7 @@ __device__ __forceinline__ void wilson_body(const EvalArgs& a, const int n_grid,
                                 const float2 u = reinterpret_cast<const float2*>(ring)[i], v = reinterpret_cast<const float2*>(ring)[i + 1];
                                 yx = u.x; yy = u.y; zx = v.x; zy = v.y;
                             }
-                        } else if (seeded) {
+                        } else if constexpr (seeded) {
                             // what wl_loops_generate stores: y - centre of mass, rounded once to the storage type
                             const double2 u = yraw[i], v = yraw[i + 1], m = sc->mean;
                             yx = u.x - m.x; yy = u.y - m.y; zx = v.x - m.x; zy = v.y - m.y;
@@ -329,29 +334,39 @@ __device__ __forceinline__ void wilson_body(const EvalArgs& a, const int n_grid,
             if (gp_ok >> j & 1) a.partial[((int64_t)v * n_units + unit) * n_grid + (a.partial_in_walk_order ? vp[j] : gp[j])] = Wsum[v][j];
 }
 
-template <class Term, bool DISC, bool BULK>
+template <class Term, bool DISC, bool BULK, bool SEEDED = false>
 __global__ void __launch_bounds__(Term::kThreads, Term::kMinBlocks)
 k_wilson(const EvalArgs a, const int n_grid, const int n_tiles, const int loops_per_unit, const int64_t n_units)
 {
-    wilson_body<Term, DISC, BULK>(a, n_grid, n_tiles, loops_per_unit, n_units);
+    wilson_body<Term, DISC, BULK, SEEDED>(a, n_grid, n_tiles, loops_per_unit, n_units);
 }
 
-// One launch of k_wilson<Term, DISC, BULK> over plan.n_units x n_tiles CTAs.
-template <class Term, bool DISC, bool BULK>
-cudaError_t launch_term(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s)
+// One launch of k_wilson<Term, DISC, BULK, SEEDED> over plan.n_units x n_tiles CTAs.
+template <class Term, bool DISC, bool BULK, bool SEEDED>
+cudaError_t launch_term_seeded(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s)
 {
     const int n_tiles = (plan.n_grid + Term::kThreads * Term::kP - 1) / (Term::kThreads * Term::kP);
-    const size_t smem = Term::stage_bytes(a.quad)
-                        + wilson_extra_smem<Term>(a.n_ppl, !DISC && !BULK && a.seeded, BULK, a.loops_are_f64 != 0);
+    const size_t smem = Term::stage_bytes(a.quad) + wilson_extra_smem<Term>(a.n_ppl, SEEDED, BULK, a.loops_are_f64 != 0);
     const int64_t n_ctas = plan.n_units * n_tiles;
     if (n_ctas > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     if (smem > 48 * 1024) {
-        cudaError_t e = cudaFuncSetAttribute(k_wilson<Term, DISC, BULK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaError_t e = cudaFuncSetAttribute(k_wilson<Term, DISC, BULK, SEEDED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    k_wilson<Term, DISC, BULK><<<(unsigned)n_ctas, Term::kThreads, smem, s>>>(a, plan.n_grid, n_tiles, plan.loops_per_unit,
-                                                                            plan.n_units);
+    k_wilson<Term, DISC, BULK, SEEDED><<<(unsigned)n_ctas, Term::kThreads, smem, s>>>(a, plan.n_grid, n_tiles,
+                                                                                    plan.loops_per_unit, plan.n_units);
     return cudaGetLastError();
+}
+
+// The seeded instantiation exists for the ordinary pass with ordinary staging only (as before, a.seeded is ignored
+// by the discretisation and bulk-staging kernels).
+template <class Term, bool DISC, bool BULK>
+cudaError_t launch_term(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s)
+{
+    if constexpr (!DISC && !BULK) {
+        if (a.seeded) return launch_term_seeded<Term, false, false, true>(plan, a, s);
+    }
+    return launch_term_seeded<Term, DISC, BULK, false>(plan, a, s);
 }
 
 // BULK staging needs whole 16-byte units: FP32 loops with an even number of points (FP64 points are 16 bytes).

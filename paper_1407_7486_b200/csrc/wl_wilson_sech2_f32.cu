@@ -40,7 +40,7 @@ cudaError_t launch_shape(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s
 
 // plan.P grid points per thread (2 or 4); grids of at most 256 points run 128 threads x 2 grid points, so that
 // no thread of the tile idles.  256 threads x P = 4 at 4 CTAs/SM (64 registers), inner loop unrolled by 2, is
-// the fastest of the combinations measured (profiles/r01_variants.md).
+// the fastest of the combinations measured (profiles/r03_wilson_f32_ncu.md, "Tried").
 cudaError_t launch_wilson_sech2_f32(const EvalPlan& plan, const EvalArgs& a, cudaStream_t s)
 {
     if (plan.n_grid <= 256) return launch_shape<2, 128>(plan, a, s);
