@@ -50,8 +50,9 @@ typedef enum {
     WL_ERR_UNSUPPORTED = 2,   /* valid request this build has no kernel for      */
     WL_ERR_WORKSPACE = 3,     /* workspace null or smaller than *_workspace_bytes */
     WL_ERR_CUDA = 4,          /* a CUDA runtime call failed (no device, launch)  */
-    WL_ERR_STATIC_LIMIT = 5   /* wl_eval_static only: the sizes need more scratch than the library's
+    WL_ERR_STATIC_LIMIT = 5,  /* wl_eval_static only: the sizes need more scratch than the library's
                                  built-in array holds (wl_eval_static_max_bytes); use wl_eval */
+    WL_ERR_NOMEM = 6          /* an allocation failed: the field object (host), wl_eval_host's buffers (device) */
 } wl_status;
 
 /* Field profiles B_z(rho), gauge A = A_phi(rho) e_phi, A_phi = Phi(rho)/(2 pi rho)
@@ -77,12 +78,13 @@ typedef enum { WL_F32 = 0, WL_F64 = 1 } wl_dtype;
 
 typedef struct wl_field wl_field;   /* opaque, host memory, immutable after creation */
 
-/* Creates a field description.  h_params: UNIFORM n_params == 1 {eB};
+/* Creates a field description: the profile B_z(rho) and its gauge potential, eq. (13)-(17).
+ * h_params: UNIFORM n_params == 1 {eB};
  * SECH2 n_params == 2 {eB0, lambda}, lambda > 0.  Non-finite values, lambda <= 0,
  * a wrong n_params or an unknown profile give WL_ERR_INVALID_ARG and *out = NULL.
  * The caller releases it with wl_field_destroy.  Host-only; no CUDA call. */
 wl_status wl_field_create(wl_profile profile, const double* h_params, int n_params, wl_field** out);
-/* Same with the particle type stated (wl_field_create = WL_FERMION); FLUXTUBE: n_params == 2,
+/* Same with the particle type stated (wl_field_create = WL_FERMION; eq. (18)); FLUXTUBE: n_params == 2,
  * {script-F, lambda}, lambda > 0.  An unknown particle gives WL_ERR_INVALID_ARG. */
 wl_status wl_field_create_particle(wl_profile profile, const double* h_params, int n_params,
                                    wl_particle particle, wl_field** out);
@@ -100,7 +102,8 @@ wl_status wl_loops_generate(void* d_loops, wl_dtype storage, int64_t loop_begin,
                             int n_ppl, uint64_t seed, void* stream);
 
 /* Bytes of device workspace wl_eval needs for these sizes (0 on invalid sizes).
- * The workspace holds per-loop-chunk partial sums; its contents are scratch. */
+ * The workspace holds the partial sums of eq. (60), one per unit of consecutive loops and grid
+ * point, which the group reduction adds in unit order; its contents are scratch. */
 size_t wl_eval_workspace_bytes(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups,
                                wl_dtype compute);
 
@@ -214,7 +217,8 @@ typedef struct wl_eval_options {
 /* Fills *opt with the defaults (= plain wl_eval).  NULL is ignored. */
 void wl_eval_options_default(wl_eval_options* opt);
 
-/* wl_eval with options (opt == NULL: exactly wl_eval).  Workspace: wl_eval_opt_workspace_bytes
+/* wl_eval with options (opt == NULL: exactly wl_eval; the options are those above: eq. (24), PAPER.md:152-168;
+ * PAPER.md:576).  Workspace: wl_eval_opt_workspace_bytes
  * (0 on invalid sizes or options).  Errors as wl_eval; an unknown quadrature order, a struct_size
  * that is not sizeof(wl_eval_options), seeded with a bad n_ppl -> WL_ERR_INVALID_ARG. */
 size_t wl_eval_opt_workspace_bytes(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups,
@@ -239,7 +243,8 @@ wl_status wl_eval_seeded(const wl_field* field, uint64_t seed, int64_t loop_begi
                          double* d_W_mean, double* d_group_sums,
                          void* d_workspace, size_t workspace_bytes, void* stream);
 
-/* wl_eval_per_loop with options (quadrature_order, seeded; shuffle_groups is ignored). */
+/* wl_eval_per_loop with options (quadrature_order, seeded; shuffle_groups is ignored): W, phase and spin of
+ * eq. (18), (21)-(24), (31)-(33), for every loop separately. */
 wl_status wl_eval_per_loop_opt(const wl_field* field,
                                const void* d_loops, wl_dtype loop_dtype, int64_t n_loops, int n_ppl,
                                const double* d_T, int n_T,
@@ -248,7 +253,7 @@ wl_status wl_eval_per_loop_opt(const wl_field* field,
                                double* d_W, double* d_phase, double* d_spin, void* stream,
                                const wl_eval_options* opt);
 
-/* The group-membership table of shuffle_groups: d_perm[t][i] = pi_t(i) (int32, [n_T][n_loops]).
+/* The group-membership table of shuffle_groups (Sec. IV.B.3; reading A17): d_perm[t][i] = pi_t(i) (int32, [n_T][n_loops]).
  * pi_t is a keyed bijection of [0, n_loops): a balanced Feistel network of 6 rounds on 2b bits (b the
  * smallest integer with 4^b >= n_loops) whose round function is word 0 of Philox4x32-10 with counter
  * (R, round, t, 0x5348464C) and key (seed_lo, seed_hi), applied again while the image is >= n_loops
@@ -268,8 +273,8 @@ wl_status wl_eval_instrumented(const wl_field* field,
                   void* d_workspace, size_t workspace_bytes, void* stream,
                   void* event_wilson_begin, void* event_wilson_end);
 
-/* Same kernels, but the per-loop values are written instead of reduced (for
- * parity triage; not part of the timed path):  d_W, d_phase, d_spin are each
+/* Same kernels, but the per-loop values W, phase, spin of eq. (18), (21)-(24), (31)-(33), PAPER.md:121-185,
+ * are written instead of reduced (for parity triage; not part of the timed path):  d_W, d_phase, d_spin are each
  * [n_loops][n_T][n_rho] FP64; d_phase / d_spin may be NULL.  No workspace. */
 wl_status wl_eval_per_loop(const wl_field* field,
                            const void* d_loops, wl_dtype loop_dtype, int64_t n_loops, int n_ppl,
@@ -335,13 +340,16 @@ wl_status wl_jackknife_finalize(const double* d_group_sums, int n_groups, int64_
                                 int n_T, int n_rho,
                                 double* d_mean, double* d_err, double* d_delete_one, void* stream);
 
-/* End-to-end convenience call on HOST buffers: allocates device memory, copies
+/* End-to-end convenience call on HOST buffers (the whole path of eq. (8)-(63), in one
+ * call): allocates device memory, copies
  * h_loops / grids to the device, runs wl_eval + wl_jackknife_finalize on an
  * internal stream (the copy of all but the first few jackknife groups overlaps the
  * evaluation of those; same bits as one wl_eval), copies h_W_mean[n_T][n_rho], h_err[n_T][n_rho]
  * and h_group_sums[G][n_T][n_rho] back, returns the device memory to the library's pool (see
  * wl_eval_host_trim) and returns after everything has completed.  h_phi_cm, h_err and h_group_sums may be NULL.
- * This is the only call that allocates, copies and synchronises. */
+ * This is the only call that allocates, copies and synchronises.  Calls on the same device are serialised
+ * (they share two internal streams); threads driving different devices run concurrently.
+ * A failed device allocation gives WL_ERR_NOMEM. */
 wl_status wl_eval_host(const wl_field* field,
                        const void* h_loops, wl_dtype loop_dtype, int64_t n_loops, int n_ppl,
                        const double* h_T, int n_T,
@@ -357,7 +365,7 @@ wl_status wl_eval_host_trim(void);
 int wl_eval_launch_count(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups,
                          wl_dtype compute);
 
-/* Static string for a status code (never NULL). */
+/* Static string for a status code (never NULL); the paper's "check the code, print the string". */
 const char* wl_status_string(wl_status status);
 
 /* "major.minor" of this ABI. */

@@ -240,6 +240,17 @@ def wl_eval_options(quadrature_order=1, seed=None, loop_begin=0, shuffle_seed=No
     return o
 
 
+def _own_options(options) -> _Options:
+    """A private copy of the caller's options block (or fresh defaults): the wrappers below set fields of it
+    (seeded, ensemble_loops, event handles) and must not leave them behind in an object the caller may reuse."""
+    o = _Options()
+    if options is None:
+        _lib.wl_eval_options_default(C.byref(o))
+    else:
+        C.memmove(C.byref(o), C.byref(options), C.sizeof(_Options))
+    return o
+
+
 def _scratch(nbytes, dev, stream):
     """Scratch bytes for kernels enqueued on `stream`: allocated under that stream, so that PyTorch's caching
     allocator does not hand the block to another stream's tensor while those kernels still use it."""
@@ -280,6 +291,7 @@ def wl_eval(field, loops, T, rho_cm, phi_cm=None, n_groups=1, compute=torch.floa
     with torch.cuda.device(dev):
         if options is not None:
             if wilson_events is not None:
+                options = _own_options(options)
                 e0, e1 = (_event_handle(ev, stream) for ev in wilson_events)
                 options.event_wilson_begin, options.event_wilson_end = e0, e1
             _check(_lib.wl_eval_opt(*args, _stream(stream), C.byref(options)), "wl_eval_opt")
@@ -336,6 +348,7 @@ def wl_eval_seeded(field, seed, n_loops, n_ppl, T, rho_cm, phi_cm=None, n_groups
         group_sums = torch.empty((n_groups, n_T, n_rho), dtype=torch.float64, device=dev)
     cc, sc = _dtype_code(compute), _dtype_code(storage)
     if options is not None:
+        options = _own_options(options)
         options.seeded, options.seed, options.loop_begin = 1, int(seed), int(loop_begin)
     if workspace is None:
         workspace = _scratch(wl_eval_opt_workspace_bytes(n_loops, n_ppl, n_T, n_rho, n_groups, cc, options), dev, stream)

@@ -14,10 +14,12 @@ bool sizes_ok(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups)
     if (n_loops % n_groups != 0) return false;                       // equal groups
     if ((int64_t)n_T * n_rho > (1 << 24)) return false;
     if (n_loops > (1LL << 40)) return false;
-    // launch limits, checked before anything is enqueued: k_wilson has at most n_loops x tiles(128 points)
-    // CTAs, the group reductions n_groups x tiles(256 points)
+    // launch limits, checked before anything is enqueued.  k_wilson: the exact CTA count (units x tiles) depends on
+    // the kernel that is dispatched and is checked by launch_term before its launch (cudaErrorInvalidConfiguration ->
+    // WL_ERR_INVALID_ARG, launch_status); here only what no kernel can launch: the largest unit is 8 loops, the
+    // largest tile 1024 grid points (256 threads x 4).  The group reductions: n_groups x tiles(256 points), exact.
     const int64_t n_grid = (int64_t)n_T * n_rho;
-    if (n_loops * ((n_grid + 127) / 128) > 0x7fffffffLL) return false;
+    if (((n_loops + 7) / 8) * ((n_grid + 1023) / 1024) > 0x7fffffffLL) return false;
     if ((int64_t)n_groups * ((n_grid + 255) / 256) > 0x7fffffffLL) return false;
     return true;
 }
@@ -77,6 +79,7 @@ wl_status launch_status(cudaError_t e)
 {
     if (e == cudaSuccess) return WL_OK;
     cudaGetLastError();
+    if (e == cudaErrorInvalidConfiguration) return WL_ERR_INVALID_ARG;     // more CTAs than a grid holds: nothing was launched
     return e == cudaErrorInvalidValue ? WL_ERR_UNSUPPORTED : WL_ERR_CUDA;
 }
 
@@ -105,7 +108,7 @@ wl_status wl_field_create_particle(wl_profile profile, const double* h_params, i
     }
     if (particle != WL_FERMION && particle != WL_SCALAR) return WL_ERR_INVALID_ARG;
     wl_field* f = new (std::nothrow) wl_field;
-    if (!f) return WL_ERR_INVALID_ARG;
+    if (!f) return WL_ERR_NOMEM;
     f->profile = (int)profile;
     f->p0 = h_params[0];
     f->p1 = (n_params > 1) ? h_params[1] : 0.0;
@@ -353,6 +356,7 @@ const char* wl_status_string(wl_status status)
         case WL_ERR_UNSUPPORTED: return "unsupported configuration";
         case WL_ERR_WORKSPACE: return "workspace missing or too small";
         case WL_ERR_CUDA: return "CUDA runtime error";
+        case WL_ERR_NOMEM: return "out of host or device memory";
         case WL_ERR_STATIC_LIMIT: return "sizes need more scratch than wl_eval_static's built-in array (wl_eval_static_max_bytes): use wl_eval with a workspace";
     }
     return "unknown status";

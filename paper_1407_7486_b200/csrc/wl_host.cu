@@ -13,13 +13,14 @@ cudaMemPool_t g_pool[64] = {};
 std::mutex g_pool_mutex;
 
 // The two streams (compute, copy) and two events of a call are created once per device and kept, like the
-// pool; g_call_mutex serialises wl_eval_host calls (they share these handles).
+// pool; g_call_mutex[device] serialises the wl_eval_host calls on one device (they share these handles), while
+// threads that drive different devices run side by side.
 struct HostHandles {
     cudaStream_t s = nullptr, copy = nullptr;
     cudaEvent_t ev[2] = {nullptr, nullptr};
 };
 HostHandles g_handles[64];
-std::mutex g_call_mutex;
+std::mutex g_call_mutex[64];
 
 cudaError_t host_handles(HostHandles** out)
 {
@@ -101,16 +102,22 @@ extern "C" wl_status wl_eval_host(const wl_field* field, const void* h_loops, wl
 
     const size_t n_grid = (size_t)n_T * n_rho;
     const size_t loop_bytes = (size_t)n_loops * n_ppl * 2 * (loop_dtype == WL_F64 ? 8 : 4);
-    DeviceBuffers d;
     enum { LOOPS, T, RHO, PHI, MEAN, GS, ERR, WS };
 #define WL_TRY(call) do { if ((call) != cudaSuccess) { cudaGetLastError(); return WL_ERR_CUDA; } } while (0)
-    std::lock_guard<std::mutex> call_lock(g_call_mutex);
+    int dev = -1;
+    WL_TRY(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return WL_ERR_CUDA;
+    // The lock is taken BEFORE the buffers exist, so that it is released AFTER ~DeviceBuffers has freed them and
+    // synchronised the two shared streams: the next caller on this device never sees this call's work in flight.
+    std::lock_guard<std::mutex> call_lock(g_call_mutex[dev]);
+    DeviceBuffers d;
     HostHandles* hh = nullptr;
     WL_TRY(host_handles(&hh));
     d.s = hh->s; d.copy = hh->copy; d.ev[0] = hh->ev[0]; d.ev[1] = hh->ev[1];
     cudaMemPool_t pool;
     WL_TRY(host_pool(&pool));
-#define WL_ALLOC(slot, bytes) WL_TRY(cudaMallocFromPoolAsync(&d.p[slot], (bytes), pool, d.s))
+#define WL_ALLOC(slot, bytes) do { const cudaError_t ea = cudaMallocFromPoolAsync(&d.p[slot], (bytes), pool, d.s); \
+        if (ea != cudaSuccess) { cudaGetLastError(); return ea == cudaErrorMemoryAllocation ? WL_ERR_NOMEM : WL_ERR_CUDA; } } while (0)
     WL_ALLOC(LOOPS, loop_bytes);
     WL_ALLOC(T, n_T * sizeof(double));
     WL_ALLOC(RHO, n_rho * sizeof(double));

@@ -73,7 +73,7 @@ def wl_eval_sharded(field, local_loops, T, rho_cm, phi_cm, shard: Shard, compute
     if local_loops.shape[0] != shard.n_loops:
         raise ValueError("local_loops has %d loops, the shard owns %d" % (local_loops.shape[0], shard.n_loops))
     # the units of loops are those of one call over the whole ensemble: same bits for any number of ranks
-    opt = options if options is not None else api.wl_eval_options()
+    opt = api._own_options(options)                    # a copy: the caller's block keeps ensemble_loops = 0
     opt.ensemble_loops = shard.n_loops * shard.world_size
     _, gs_local = api.wl_eval(field, local_loops, T, rho_cm, phi_cm, n_groups=shard.n_groups, compute=compute,
                               stream=stream, workspace=workspace, options=opt)

@@ -35,9 +35,29 @@ def test_library_exports_every_declared_symbol(lib):
         assert hasattr(lib, name), name
 
 
+HOUSEKEEPING = {"wl_field_destroy", "wl_eval_options_default", "wl_eval_host_trim", "wl_eval_launch_count", "wl_version"}
+
+
 def test_every_declared_call_cites_the_paper():
+    """Each prototype's own comment (the block comment that precedes it) names the passage that defines the
+    operation: a PAPER.md line, or the DESIGN.md reading / SURVEY.md section that stands for it.  Calls that
+    compute nothing of the method (HOUSEKEEPING) are exempt."""
     src = open(HEADER).read()
-    assert src.count("PAPER.md:") >= 10
+    comment, uncited, seen = None, [], set()
+    for m in re.finditer(r"/\*.*?\*/|\b(wl_[a-z_0-9]+)\s*\(", src, flags=re.S):
+        if m.group(0).startswith("/*"):
+            line_start = src.rfind("\n", 0, m.start()) + 1
+            if src[line_start:m.start()].strip() == "":           # a block comment of its own, not a trailing remark
+                comment = m.group(0)
+            continue
+        name = m.group(1)
+        seen.add(name)
+        if name in HOUSEKEEPING:
+            continue
+        if not (comment and ("PAPER.md:" in comment or "DESIGN.md" in comment or "SURVEY.md" in comment)):
+            uncited.append(name)
+    assert not uncited, uncited
+    assert seen == set(declared_symbols())
 
 
 def test_field_create_validation(lib):
@@ -73,8 +93,8 @@ def test_field_create_validation(lib):
 
 def test_status_strings(lib):
     lib.wl_status_string.restype = C.c_char_p
-    seen = {lib.wl_status_string(i) for i in range(5)}
-    assert len(seen) == 5 and all(seen)
+    seen = {lib.wl_status_string(i) for i in range(7)}
+    assert len(seen) == 7 and all(seen)
     assert lib.wl_status_string(99)
 
 
@@ -94,6 +114,10 @@ def test_workspace_plan_is_a_function_of_sizes_only(lib):
     assert f(0, 64, 4, 4, 1, 0) == 0
     assert f(8, 64, 0, 4, 1, 0) == 0
     assert f(8, 64, 4, 4, 1, 5) == 0
+    # the CTA bound follows the real launch shape: 2^24 loops on a 128 x 128 grid are 2^21 units x 16 tiles = 2^25 CTAs
+    assert f(1 << 24, 64, 128, 128, 16, 0) == (1 << 21) * 128 * 128 * 8
+    # ... and what no kernel shape can launch is refused: 2^40 loops x 4 tiles of 1024 points, in units of 8
+    assert f(1 << 40, 64, 64, 64, 16, 0) == 0
 
 
 def test_compute_calls_reject_bad_arguments_without_a_gpu(lib):
@@ -192,3 +216,16 @@ def test_grid_validate_and_permutation_argument_checks(lib):
     assert lib.wl_group_permutation(1, 8, 4, None, None) == 1
     lib.wl_version.restype = C.c_char_p
     assert lib.wl_version() == b"2.0"
+
+
+def test_binding_never_writes_into_the_callers_options_block():
+    """api.wl_eval_seeded / wl_eval(wilson_events=...) / shard.wl_eval_sharded set fields (seeded, event handles,
+    ensemble_loops) on a private copy: a block the caller reuses for a later plain call keeps its own values."""
+    from paper_1407_7486_b200 import api
+    mine = api.wl_eval_options(quadrature_order=2, shuffle_seed=5)
+    copy = api._own_options(mine)
+    copy.ensemble_loops, copy.seeded, copy.seed = 99, 1, 7
+    assert (mine.ensemble_loops, mine.seeded, mine.seed) == (0, 0, 0)
+    assert (copy.quadrature_order, copy.shuffle_groups, copy.shuffle_seed, copy.struct_size) == (2, 1, 5, mine.struct_size)
+    fresh = api._own_options(None)
+    assert fresh.quadrature_order == 1 and fresh.struct_size == mine.struct_size and fresh.seeded == 0

@@ -199,6 +199,36 @@ def test_host_call_equals_device_call(api):
     api.wl_eval_host_trim()
 
 
+def test_host_calls_from_two_threads_on_one_device_serialise(api):
+    """wl_eval_host shares two streams and a pool per device: concurrent callers on that device take turns
+    (one mutex per device) and each gets the result of its own inputs."""
+    import threading
+    c = inputs.config(1)
+    T, rho, _ = c.grids()
+    f = api.wl_field_create(c.profile, c.params)
+    ys = [api.wl_loops_generate(128, c.n_ppl, seed, torch.float32).cpu().numpy() for seed in (11, 12, 13, 14)]
+    want = [api.wl_eval_host(f, y, T, rho, None, n_groups=8, compute="f32") for y in ys]
+    got, errors = [None] * len(ys), []
+
+    def work(k):
+        try:
+            torch.cuda.set_device(0)
+            for _ in range(3):
+                got[k] = api.wl_eval_host(f, ys[k], T, rho, None, n_groups=8, compute="f32")
+        except Exception as exc:                       # surfaced in the main thread below
+            errors.append(exc)
+
+    threads = [threading.Thread(target=work, args=(k,)) for k in range(len(ys))]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+    for (m, e, g), (wm, we, wg) in zip(got, want):
+        assert np.array_equal(m, wm) and np.array_equal(e, we) and np.array_equal(g, wg)
+    assert not np.array_equal(want[0][0], want[1][0])
+
+
 def test_error_statuses(api):
     loops = api.wl_loops_generate(8, 16, 1, torch.float64)
     f = api.wl_field_create(inputs.SECH2, (1.0, 1.0))
