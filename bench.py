@@ -152,17 +152,150 @@ def base_line(args, cfg, n_gpus):
     }
 
 
-def workload_config(cfg, n_gpus, compute):
+def workload_config(cfg, n_gpus):
     return {
         "workload": cfg.name,
         "n_loops_per_gpu": cfg.n_loops, "n_loops_total": cfg.n_loops * n_gpus, "n_ppl": cfg.n_ppl,
         "n_T": cfg.n_T, "n_rho": cfg.n_rho, "n_groups_total": cfg.n_groups * n_gpus,
         "field": {"profile": "sech2" if cfg.profile == 1 else "uniform", "params": list(cfg.params)},
-        "loop_storage": cfg.loop_dtype, "compute": compute, "seed": cfg.seed,
+        "loop_storage": cfg.loop_dtype, "seed": cfg.seed,
         "parallelism": "dp%d (whole jackknife groups per rank)" % n_gpus,
         "cache": "inputs larger than L2 (%.0f MB of loop coordinates per step vs 126 MB L2)"
                  % (cfg.n_loops * cfg.n_ppl * 2 * (4 if cfg.loop_dtype == "f32" else 8) / 1e6),
     }
+
+
+def kernel_sfu_ops(n_grid, has_phi, Q, scalar=False):
+    """MUFU instructions per point-eval of k_wilson<Sech2PackedF32>, from the predicates the dispatcher uses
+    (wl_wilson_sech2_f32.cu, wl_terms_packed_f32.cuh): sqrt, rsqrt and two ex2 at the midpoint rule (the scalar-only
+    variant, which has no spin sum, issues 2), + 2 per further Gauss-Legendre node; the one reciprocal
+    per staged point and thread is shared by the P grid points of the thread and is a MUFU unless kFmaRcp
+    (= fermion loops, no phi_cm, 256-thread tiles) puts it on the FMA pipe."""
+    threads = 128 if n_grid <= 256 else 256
+    P = 4 if (n_grid >= 1024 and Q == 1) else 2
+    fma_rcp = (not scalar) and (not has_phi) and threads >= 256
+    base = 2 if scalar else KERNEL_SFU_OPS
+    return base + 2 * (Q - 1) + (0.0 if fma_rcp else 1.0 / P)
+
+
+def kernel_roofline(cfg, compute, Q, has_phi, sm_max_mhz):
+    """(algorithmic lane-ops per point-eval, how counted, peak lane-ops/s, how derived, pipe_frac or None) of the
+    k_wilson instantiation that serves (cfg, compute, Q): DESIGN.md section 5."""
+    pipe_frac = None          # the binding pipe's utilisation by the instructions the kernel really issues
+    if compute == "f32":
+        if cfg.profile == 1:
+            ops = ALG_PLAIN_OPS + ALG_SFU_OPS + (Q - 1) * (ALG_NODE_PLAIN_OPS + ALG_NODE_SFU_OPS)
+            ops_how = ("%d algorithmic FP32 lane-ops per point-eval (29 plain + 7 special-function, SURVEY.md 8(d)%s)"
+                       % (ops, "" if Q == 1 else "; + 11 + 2 per extra Gauss-Legendre node"))
+            pipe_frac = {"pipe": "xu", "ops_per_point_eval": kernel_sfu_ops(cfg.n_T * cfg.n_rho, has_phi, Q),
+                         "peak_lanes_per_clk_sm": SFU_LANES_PER_CLK_SM}
+        else:
+            ops = ALG_OPS_UNIFORM
+            ops_how = "%d algorithmic FP32 lane-ops per point-eval (uniform field: the bare cross product)" % ops
+        peak = SM_COUNT * ISSUE_LANES_PER_CLK_SM * sm_max_mhz * 1e6
+        peak_how = ("derived: 148 SMs x 4 sub-partitions x 32 lanes x %d MHz (FP32 non-tensor issue roofline, the "
+                    "north_star denominator; FFMA micro-benchmark measured 123-127 of 128 lanes/clk/SM, "
+                    "profiles/r01_pipe_rates.md). Packed FFMA2 does not raise the FMA-pipe rate; XU and ALU-pipe work "
+                    "can overlap it, so the binding pipe's own utilisation is given in pipe_frac" % sm_max_mhz)
+    else:
+        if cfg.profile == 1:
+            ops = ALG_F64_OPS_SECH2
+            ops_how = ("%d FP64 lane-ops per point-eval counted from the mathematics (29 plain + 55 for the seven "
+                       "elementary functions as shortest double-precision sequences, the logarithm at the degree it needs "
+                       "far from the axis; DESIGN.md section 5)" % ops)
+            if Q == 1:
+                pipe_frac = {"pipe": "fp64", "ops_per_point_eval": KERNEL_F64_OPS_SECH2,
+                             "peak_lanes_per_clk_sm": FP64_LANES_PER_CLK_SM}
+        else:
+            ops = ALG_OPS_UNIFORM
+            ops_how = "%d algorithmic FP64 lane-ops per point-eval (uniform field)" % ops
+        peak = SM_COUNT * FP64_LANES_PER_CLK_SM * sm_max_mhz * 1e6
+        peak_how = "derived: 148 SMs x 64 FP64 lanes x %d MHz (DFMA micro-benchmark measured 62-63.8 of 64)" % sm_max_mhz
+    return ops, ops_how, peak, peak_how, pipe_frac
+
+
+def finish_pipe_frac(pipe_frac, evals, k_ms, sm_max_mhz):
+    if pipe_frac is None:
+        return
+    pipe_frac["frac"] = (pipe_frac["ops_per_point_eval"] * evals / (k_ms * 1e-3)) / (
+        SM_COUNT * pipe_frac["peak_lanes_per_clk_sm"] * sm_max_mhz * 1e6)
+    pipe_frac["note"] = ("instructions the kernel issues on its binding pipe (not an algorithmic count)"
+                         + ("; the count of the farthest tier, tier 0 issues 97: a lower bound of the utilisation"
+                            if pipe_frac["pipe"] == "fp64" else ""))
+
+
+def time_secondary(api, cfg, compute, steps, warmup, sm_max_mhz):
+    """One of the other BASELINE.json configs under the same clock as the headline: device-resident loops, wl_eval +
+    wl_jackknife_finalize per step, CUDA events on the launching stream around the steps and around k_wilson."""
+    import torch
+    T, rho, phi = cfg.grids()
+    dev = lambda a: torch.tensor(a, dtype=torch.float64, device="cuda") if a is not None else None
+    Td, rd, pd = dev(T), dev(rho), dev(phi)
+    field = api.wl_field_create(cfg.profile, cfg.params)
+    tdt = torch.float32 if cfg.loop_dtype == "f32" else torch.float64
+    loops = api.wl_loops_generate(cfg.n_loops, cfg.n_ppl, cfg.seed, tdt)
+    ws = api.wl_eval_workspace_bytes(cfg.n_loops, cfg.n_ppl, cfg.n_T, cfg.n_rho, cfg.n_groups, compute)
+    workspace = torch.empty(max(ws, 8), dtype=torch.uint8, device="cuda")
+    W_mean = torch.empty((cfg.n_T, cfg.n_rho), dtype=torch.float64, device="cuda")
+    gs = torch.empty((cfg.n_groups, cfg.n_T, cfg.n_rho), dtype=torch.float64, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def step(events=None):
+        api.wl_eval(field, loops, Td, rd, pd, n_groups=cfg.n_groups, compute=compute, W_mean=W_mean, group_sums=gs,
+                    workspace=workspace, wilson_events=events)
+        return api.wl_jackknife_finalize(gs, cfg.n_loops)
+
+    for _ in range(warmup):
+        step()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for a, b in ev:
+        a.record(stream)
+        b.record(stream)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler = ClockSampler(nvml_index_for(torch.cuda.current_device()))
+    torch.cuda.synchronize()
+    sampler.start()
+    e0.record(stream)
+    for k in range(steps):
+        mean, _ = step(ev[k])
+    e1.record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1) / steps
+    k_ms = sum(a.elapsed_time(b) for a, b in ev) / steps
+    checksum = float(mean.sum().item())
+    ops, _, peak, _, pipe_frac = kernel_roofline(cfg, compute, 1, phi is not None, sm_max_mhz)
+    finish_pipe_frac(pipe_frac, cfg.point_evals, k_ms, sm_max_mhz)
+    return {"workload": cfg.name, "dtype": compute, "steps": steps, "warmup": warmup,
+            "value": cfg.point_evals / (ms * 1e-3), "ms_per_step": ms, "kernel_ms": k_ms,
+            "frac": ops * cfg.point_evals / (k_ms * 1e-3) / peak,
+            "pipe_frac": ({"pipe": pipe_frac["pipe"], "frac": pipe_frac["frac"]} if pipe_frac else None),
+            "clocks": clocks, "checksum_sum_W_mean": checksum,
+            "cache": "%.0f MB of loop coordinates per step%s" % (
+                loops.numel() * loops.element_size() / 1e6,
+                "" if loops.numel() * loops.element_size() > 126e6 else " (smaller than the 126 MB L2: L2-resident between steps)")}
+
+
+def run_secondary(api, headline_workload, sm_max_mhz):
+    """The other configs of BASELINE.json, 2 timed steps each after 1 warm-up step (the FP64 leg of config 4 takes
+    ~8 s per step), so that every configuration north_star names is timed by the same run as the headline."""
+    import torch
+    from paper_1407_7486_b200 import inputs
+    out = []
+    for number in (4, 5, 2, 1):
+        cfg = inputs.config(number)
+        for compute in ("f32", "f64"):
+            if compute not in cfg.compute and not (number == 1 and compute == "f32"):
+                continue
+            if number == headline_workload:
+                continue
+            steps, warmup = (2, 1) if number in (4, 5) else (5, 3)
+            try:
+                out.append(time_secondary(api, cfg, compute, steps, warmup, sm_max_mhz))
+            except Exception as exc:                      # the headline line must still be printed
+                out.append({"workload": cfg.name, "dtype": compute, "error": "%s: %s" % (type(exc).__name__, exc)})
+            torch.cuda.empty_cache()
+    return out
 
 
 def run_reference(args, cfg):
@@ -189,7 +322,7 @@ def run_reference(args, cfg):
     line = base_line(args, cfg, args.gpus)
     line.update({
         "impl": "reference", "value": value, "ms_per_step": 1e3 * total_t / args.steps, "dtype": "f64",
-        "config": workload_config(cfg, 1, "f64 (oracle)"),
+        "config": workload_config(cfg, args.gpus),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0, "scaling": "weak",
@@ -340,44 +473,9 @@ def run_ours(args, cfg):
     sm_max_mhz = clocks.get("sm_max_mhz") or 1965
     k_ms = sum(wilson_ms) / len(wilson_ms)
     Q = args.quadrature
-    pipe_frac = None          # the binding pipe's utilisation by the instructions the kernel really issues
-    if compute == "f32":
-        if cfg.profile == 1:
-            ops = ALG_PLAIN_OPS + ALG_SFU_OPS + (Q - 1) * (ALG_NODE_PLAIN_OPS + ALG_NODE_SFU_OPS)
-            ops_how = ("%d algorithmic FP32 lane-ops per point-eval (29 plain + 7 special-function, SURVEY.md 8(d)%s)"
-                       % (ops, "" if Q == 1 else "; + 11 + 2 per extra Gauss-Legendre node"))
-            small = cfg.n_T * cfg.n_rho <= 256 or cfg.circle_radius is not None   # 128-thread or phi_cm kernel: MUFU reciprocal
-            pipe_frac = {"pipe": "xu", "ops_per_point_eval": KERNEL_SFU_OPS + 2 * (Q - 1) + (0.5 if small else 0.0),
-                         "peak_lanes_per_clk_sm": SFU_LANES_PER_CLK_SM}
-        else:
-            ops = ALG_OPS_UNIFORM
-            ops_how = "%d algorithmic FP32 lane-ops per point-eval (uniform field: the bare cross product)" % ops
-        peak = SM_COUNT * ISSUE_LANES_PER_CLK_SM * sm_max_mhz * 1e6
-        peak_how = ("derived: 148 SMs x 4 sub-partitions x 32 lanes x %d MHz (FP32 non-tensor issue roofline, the "
-                    "north_star denominator; FFMA micro-benchmark measured 123-127 of 128 lanes/clk/SM, "
-                    "profiles/r01_pipe_rates.md). Packed FFMA2 does not raise the FMA-pipe rate; XU and ALU-pipe work "
-                    "can overlap it, so the binding pipe's own utilisation is given in pipe_frac" % sm_max_mhz)
-    else:
-        if cfg.profile == 1:
-            ops = ALG_F64_OPS_SECH2
-            ops_how = ("%d FP64 lane-ops per point-eval counted from the mathematics (29 plain + 55 for the seven "
-                       "elementary functions as shortest double-precision sequences, the logarithm at the degree it needs "
-                       "far from the axis; DESIGN.md section 5)" % ops)
-            if Q == 1:
-                pipe_frac = {"pipe": "fp64", "ops_per_point_eval": KERNEL_F64_OPS_SECH2,
-                             "peak_lanes_per_clk_sm": FP64_LANES_PER_CLK_SM}
-        else:
-            ops = ALG_OPS_UNIFORM
-            ops_how = "%d algorithmic FP64 lane-ops per point-eval (uniform field)" % ops
-        peak = SM_COUNT * FP64_LANES_PER_CLK_SM * sm_max_mhz * 1e6
-        peak_how = "derived: 148 SMs x 64 FP64 lanes x %d MHz (DFMA micro-benchmark measured 62-63.8 of 64)" % sm_max_mhz
+    ops, ops_how, peak, peak_how, pipe_frac = kernel_roofline(cfg, compute, Q, phi is not None, sm_max_mhz)
     achieved = ops * evals_per_gpu / (k_ms * 1e-3)
-    if pipe_frac is not None:
-        pipe_frac["frac"] = (pipe_frac["ops_per_point_eval"] * evals_per_gpu / (k_ms * 1e-3)) / (
-            SM_COUNT * pipe_frac["peak_lanes_per_clk_sm"] * sm_max_mhz * 1e6)
-        pipe_frac["note"] = ("instructions the kernel issues on its binding pipe (not an algorithmic count)"
-                             + ("; the count of the farthest tier, tier 0 issues 97: a lower bound of the utilisation"
-                                if pipe_frac["pipe"] == "fp64" else ""))
+    finish_pipe_frac(pipe_frac, evals_per_gpu, k_ms, sm_max_mhz)
     traffic, traffic_note = ncu_traffic(cfg.name, compute, args)
     roofline = {
         "bound": "alu", "kernel": "k_wilson", "achieved": achieved / 1e12, "peak": peak / 1e12,
@@ -386,7 +484,15 @@ def run_ours(args, cfg):
         "algorithmic_ops": ops_how, "peak_source": peak_how, "pipe_frac": pipe_frac,
         "xu_pipe_frac": pipe_frac["frac"] if (pipe_frac and pipe_frac["pipe"] == "xu") else None,
         "fp64_pipe_frac": pipe_frac["frac"] if (pipe_frac and pipe_frac["pipe"] == "fp64") else None,
-        "algorithmic_bytes": (0 if seeded else loop_bytes) + ws_bytes,
+        "frac_meaning": ("algorithmic lane-ops per point-eval (a count from the mathematics, not of issued instructions) "
+                         "x point-evals/s over the issue peak; the utilisation figure is pipe_frac (instructions the "
+                         "kernel issues on its binding pipe over that pipe's rate)"),
+        # what the method needs: the ensemble read once + <W> and the group sums written once; the
+        # per-unit partial sums (written by k_wilson, read by k_group_reduce) are this design's workspace, stated apart
+        "algorithmic_bytes": (0 if seeded else loop_bytes) + 8 * cfg.n_T * cfg.n_rho * (1 + sh.n_groups),
+        "workspace_bytes": ws_bytes,
+        "traffic_over_algorithmic": (traffic / ((0 if seeded else loop_bytes) + 8 * cfg.n_T * cfg.n_rho * (1 + sh.n_groups))
+                                     if traffic else None),
         "hbm_GBps_algorithmic": (0 if seeded else loop_bytes) / (k_ms * 1e-3) / 1e9,
     }
 
@@ -403,15 +509,23 @@ def run_ours(args, cfg):
 
     launches_per_step = (api.wl_eval_launch_count(sh.n_loops, cfg.n_ppl, cfg.n_T, cfg.n_rho, sh.n_groups, compute) + 1
                          + (1 if args.shuffle else 0))      # + k_jackknife_finalize (+ k_group_permutation)
+    secondary = None
+    if plain and world == 1 and not args.no_secondary and args.workload == 3 and cfg.name == "cfg3_paper_scale":
+        del loops, workspace
+        torch.cuda.empty_cache()
+        secondary = run_secondary(api, args.workload, sm_max_mhz)
     line = base_line(args, cfg, world)
     line.update({
         "value": value, "ms_per_step": ms_per_step, "dtype": compute,
-        "config": dict(workload_config(cfg, world, compute), loops=args.loops, quadrature_order=args.quadrature,
-                       shuffled_groups=bool(args.shuffle), staging=args.staging),
+        "config": workload_config(cfg, world),
+        "options": {"loops": args.loops, "quadrature_order": args.quadrature, "shuffled_groups": bool(args.shuffle),
+                    "staging": args.staging},
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps,
         "roofline": roofline, "cpu_baseline": cpu_baseline,
         "checksum_sum_W_mean": result_checksum,
     })
+    if secondary is not None:
+        line["secondary"] = secondary
     print(json.dumps(line), flush=True)
     if use_dist:
         dist.barrier()
@@ -442,7 +556,7 @@ def source_sha16():
 
 def ncu_traffic(workload, compute, args):
     """dram__bytes_read.sum + dram__bytes_write.sum of one k_wilson launch, from profiles/ncu_traffic.json
-    (written by `python -m paper_1407_7486_b200.ncu_summary` from an `ncu --set full` capture).  null unless the
+    (written by `python bench.py --ncu-summary REPORT --key ...` from an `ncu --set full` capture).  null unless the
     capture was taken on exactly these kernel sources and this (workload, compute, options)."""
     path = os.path.join(ROOT, "profiles", "ncu_traffic.json")
     try:
@@ -477,12 +591,28 @@ def main():
     ap.add_argument("--n-loops", type=int, default=None, help="override the workload's loops per GPU (a multiple of its groups)")
     ap.add_argument("--loop-dtype", choices=("f32", "f64"), default=None, help="override the loop storage precision")
     ap.add_argument("--source-sha", action="store_true", help="print the hash of the kernel sources and exit")
+    ap.add_argument("--ncu-summary", metavar="REPORT", default=None,
+                    help="no benchmark: summarise an `ncu --set full` report of k_wilson as a markdown table and, with --key, "
+                         "record its DRAM bytes in profiles/ncu_traffic.json (bench_ncu_summary.py; no GPU needed)")
+    ap.add_argument("--key", default=None, help="with --ncu-summary: entry of profiles/ncu_traffic.json, e.g. cfg3_paper_scale/f32")
+    ap.add_argument("--sha", default=None, help="with --ncu-summary: source hash at capture time (--source-sha on the GPU box)")
+    ap.add_argument("--md", default=None, help="with --ncu-summary: also append the table to this file")
+    ap.add_argument("--kernel", default="k_wilson", help="with --ncu-summary: kernel name filter")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-secondary", action="store_true",
+                    help="skip the `secondary` block (configs 4, 5, 2, 1 timed after the config-3 headline)")
     args = ap.parse_args()
     if args.source_sha:
         print(source_sha16())
         return 0
+    if args.ncu_summary:
+        import bench_ncu_summary
+        argv = [args.ncu_summary, "--kernel", args.kernel]
+        for flag, val in (("--key", args.key), ("--sha", args.sha), ("--md", args.md)):
+            if val:
+                argv += [flag, val]
+        return bench_ncu_summary.main(argv)
     if args.steps < 1 or args.warmup < 0:
         raise SystemExit("--steps >= 1, --warmup >= 0")
     from paper_1407_7486_b200 import inputs

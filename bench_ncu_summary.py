@@ -1,6 +1,8 @@
 """Summarise an `ncu --set full` capture of k_wilson and record its DRAM traffic for bench.py.
 
-    python -m paper_1407_7486_b200.ncu_summary REPORT.ncu-rep --key cfg3_paper_scale/f32 [--sha SHA16] [--md OUT.md]
+    python bench.py --ncu-summary REPORT.ncu-rep --key cfg3_paper_scale/f32 [--sha SHA16] [--md OUT.md]
+
+(a mode of bench.py, which owns profiles/ncu_traffic.json; this module sits beside it and is not part of the library).
 
 Reads the report with `ncu -i REPORT --page raw --csv` (no GPU needed), prints a markdown table of the
 counters DESIGN.md section 5 argues from (pipe utilisation, issue rate, stall reasons, registers, DRAM bytes) for
@@ -17,7 +19,7 @@ import os
 import subprocess
 import sys
 
-ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+ROOT = os.path.dirname(os.path.abspath(__file__))
 
 METRICS = [
     ("gpu__time_duration.sum", "kernel time"),
@@ -43,13 +45,35 @@ METRICS = [
     ("sass__inst_executed_local_loads", "local-memory (spill) loads"),
     ("sass__inst_executed_local_stores", "local-memory (spill) stores"),
     ("l1tex__data_bank_conflicts_pipe_lsu_mem_shared.sum", "shared-memory bank conflicts"),
+    # executed lane-ops in ncu's own words (thread-level, predicated-off lanes not counted)
+    ("smsp__sass_thread_inst_executed_op_fp32_pred_on.sum", "FP32 thread instructions (FADD + FMUL + FFMA; a packed instruction counts once per half)"),
+    ("smsp__sass_thread_inst_executed_op_ffma_pred_on.sum", "... of which FFMA"),
+    ("smsp__sass_thread_inst_executed_op_fmul_pred_on.sum", "... of which FMUL"),
+    ("smsp__sass_thread_inst_executed_op_fadd_pred_on.sum", "... of which FADD"),
+    ("smsp__sass_thread_inst_executed_op_fp64_pred_on.sum", "FP64 thread instructions"),
+    ("sm__inst_executed_pipe_xu.sum", "XU-pipe warp instructions"),
+    ("sm__inst_executed_pipe_fma.sum", "FMA-pipe warp instructions"),
+    ("smsp__thread_inst_executed.sum", "thread instructions, all kinds"),
 ]
+
+# Derived: executed FP32 flops-style lane-ops per second (FFMA counted once, as one lane-op) against the issue peak
+PEAK_LANES_PER_CLK = 148 * 128
 STALL = "smsp__average_warps_issue_stalled_"
 
 
 def to_bytes(value, unit):
     scale = {"byte": 1, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}.get(unit, 1)
     return int(round(float(value.replace(",", "")) * scale))
+
+
+def to_seconds(value, unit):
+    scale = {"s": 1.0, "ms": 1e-3, "us": 1e-6, "ns": 1e-9, "second": 1.0, "msecond": 1e-3, "usecond": 1e-6, "nsecond": 1e-9}[unit]
+    return float(value.replace(",", "")) * scale
+
+
+def to_hz(value, unit):
+    scale = {"hz": 1.0, "Khz": 1e3, "Mhz": 1e6, "Ghz": 1e9}[unit]
+    return float(value.replace(",", "")) * scale
 
 
 def read_report(path):
@@ -92,6 +116,20 @@ def main(argv=None):
                     continue
                 if v >= 0.1 and "selected" not in h[len(STALL):].replace("not_selected", ""):
                     stalls.append((v, h[len(STALL):-len("_per_issue_active.ratio")]))
+        try:                                             # executed lane-op rates, beside the algorithmic count of bench.py
+            secs = to_seconds(r[col["gpu__time_duration.sum"]], units[col["gpu__time_duration.sum"]])
+            hz = to_hz(r[col["sm__cycles_elapsed.avg.per_second"]], units[col["sm__cycles_elapsed.avg.per_second"]])
+            num = lambda m: float(r[col[m]].replace(",", ""))
+            fp32 = num("smsp__sass_thread_inst_executed_op_fp32_pred_on.sum")
+            xu = num("sm__inst_executed_pipe_xu.sum") * 32.0
+            allt = num("smsp__thread_inst_executed.sum")
+            peak = PEAK_LANES_PER_CLK * hz
+            lines.append("")
+            lines.append("Executed lane-ops per second over the issue peak (148 SMs x 128 lanes x %.3f GHz = %.2f Tlane-op/s): "
+                         "FP32 arithmetic %.3f, + XU-pipe lanes %.3f, all thread instructions %.3f."
+                         % (hz / 1e9, peak / 1e12, fp32 / secs / peak, (fp32 + xu) / secs / peak, allt / secs / peak))
+        except (KeyError, ValueError):
+            pass
         stalls.sort(reverse=True)
         lines.append("")
         lines.append("Warp stalls per issue-active cycle: " + ", ".join("`%s` %.2f" % (n, v) for v, n in stalls))
@@ -111,7 +149,7 @@ def main(argv=None):
                 tab = json.load(fh)
         except (OSError, ValueError):
             tab = {"what": "dram__bytes_read.sum / dram__bytes_write.sum of one k_wilson launch per (workload/compute[/options]) "
-                           "from ncu --set full captures; written by python -m paper_1407_7486_b200.ncu_summary", "entries": {}}
+                           "from ncu --set full captures; written by python bench.py --ncu-summary", "entries": {}}
         i_r, i_w = col["dram__bytes_read.sum"], col["dram__bytes_write.sum"]
         tab["entries"][args.key] = {
             "dram_bytes_read": to_bytes(r[i_r], units[i_r]), "dram_bytes_write": to_bytes(r[i_w], units[i_w]),

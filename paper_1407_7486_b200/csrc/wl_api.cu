@@ -362,6 +362,6 @@ const char* wl_status_string(wl_status status)
     return "unknown status";
 }
 
-const char* wl_version(void) { return "2.0"; }
+const char* wl_version(void) { return "2.1"; }
 
 }  // extern "C"

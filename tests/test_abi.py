@@ -215,7 +215,7 @@ def test_grid_validate_and_permutation_argument_checks(lib):
     assert lib.wl_group_permutation(1, 8, 0, dummy, None) == 1
     assert lib.wl_group_permutation(1, 8, 4, None, None) == 1
     lib.wl_version.restype = C.c_char_p
-    assert lib.wl_version() == b"2.0"
+    assert lib.wl_version() == b"2.1"
 
 
 def test_binding_never_writes_into_the_callers_options_block():
