@@ -224,6 +224,43 @@ def finish_pipe_frac(pipe_frac, evals, k_ms, sm_max_mhz):
                             if pipe_frac["pipe"] == "fp64" else ""))
 
 
+def measure_pipe_peaks(api):
+    """The three pipe rates the rooflines rest on, measured now on this GPU: wl_pipe_probe (csrc/wl_pipe_probe.cu)
+    issues nothing but scalar FFMA / MUFU.EX2 / DFMA; each is timed with CUDA events on the launching stream (2 warm-up,
+    5 timed launches of ~17 ms, the median taken) while NVML samples the SM clock."""
+    import torch
+    sink = torch.zeros(4, dtype=torch.float32, device="cuda")
+    stream = torch.cuda.current_stream()
+    out = {}
+    sampler = ClockSampler(nvml_index_for(torch.cuda.current_device()))
+    sampler.start()
+    raw = {}
+    for pipe, name, iters in ((0, "ffma", 32768), (1, "xu_ex2", 4096), (2, "dfma", 16384)):
+        for _ in range(2):
+            lane_ops, sms = api.wl_pipe_probe(pipe, iters, sink)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(5)]
+        torch.cuda.synchronize()
+        for a, b in ev:
+            a.record(stream)
+            api.wl_pipe_probe(pipe, iters, sink)
+            b.record(stream)
+        torch.cuda.synchronize()
+        ms = sorted(a.elapsed_time(b) for a, b in ev)[2]
+        raw[name] = (lane_ops, sms, ms)
+    clocks = sampler.stop()
+    mhz = clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965
+    for name, (lane_ops, sms, ms) in raw.items():
+        out[name + "_lanes_per_clk_sm"] = lane_ops / (ms * 1e-3) / (mhz * 1e6) / sms
+        out[name + "_Tlane_ops_per_s"] = lane_ops / (ms * 1e-3) / 1e12
+    out["sm_mhz"] = mhz
+    out["clocks"] = clocks
+    out["how"] = ("wl_pipe_probe: 4 CTAs x 256 threads per SM, 16 independent chains x 8 per loop iteration of scalar FFMA / "
+                  "MUFU.EX2 / DFMA only; CUDA events, median of 5 launches; lanes per clock and SM at the NVML-sampled SM clock. "
+                  "Nominal: 128 / 16 / 64. The roofline denominators stay the derived ones (nominal lanes x max clock), "
+                  "which are the larger, i.e. `frac` is not flattered by a low measurement")
+    return out
+
+
 def time_secondary(api, cfg, compute, steps, warmup, sm_max_mhz):
     """One of the other BASELINE.json configs under the same clock as the headline: device-resident loops, wl_eval +
     wl_jackknife_finalize per step, CUDA events on the launching stream around the steps and around k_wilson."""
@@ -509,6 +546,11 @@ def run_ours(args, cfg):
 
     launches_per_step = (api.wl_eval_launch_count(sh.n_loops, cfg.n_ppl, cfg.n_T, cfg.n_rho, sh.n_groups, compute) + 1
                          + (1 if args.shuffle else 0))      # + k_jackknife_finalize (+ k_group_permutation)
+    if not args.no_pipe_peaks:
+        try:
+            roofline["peak_measured"] = measure_pipe_peaks(api)
+        except Exception as exc:                          # the headline line must still be printed
+            roofline["peak_measured"] = {"error": "%s: %s" % (type(exc).__name__, exc)}
     secondary = None
     if plain and world == 1 and not args.no_secondary and args.workload == 3 and cfg.name == "cfg3_paper_scale":
         del loops, workspace
@@ -600,6 +642,9 @@ def main():
     ap.add_argument("--kernel", default="k_wilson", help="with --ncu-summary: kernel name filter")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--pipe-peaks", action="store_true",
+                    help="no benchmark: measure the FFMA / MUFU / DFMA pipe rates with wl_pipe_probe and print them as one JSON line")
+    ap.add_argument("--no-pipe-peaks", action="store_true", help="leave roofline.peak_measured out of the line")
     ap.add_argument("--no-secondary", action="store_true",
                     help="skip the `secondary` block (configs 4, 5, 2, 1 timed after the config-3 headline)")
     args = ap.parse_args()
@@ -613,6 +658,14 @@ def main():
             if val:
                 argv += [flag, val]
         return bench_ncu_summary.main(argv)
+    if args.pipe_peaks:
+        import torch
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py --pipe-peaks: no CUDA device")
+        from paper_1407_7486_b200 import api
+        torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+        print(json.dumps({"pipe_peaks": measure_pipe_peaks(api)}), flush=True)
+        return 0
     if args.steps < 1 or args.warmup < 0:
         raise SystemExit("--steps >= 1, --warmup >= 0")
     from paper_1407_7486_b200 import inputs

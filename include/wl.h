@@ -361,6 +361,15 @@ wl_status wl_eval_host(const wl_field* field,
  * calls; this returns the pool's unused memory to the device.  WL_OK if there is nothing to release. */
 wl_status wl_eval_host_trim(void);
 
+/* Measurement helper ("rooflines"; not part of the method): enqueues on `stream` one kernel
+ * (4 CTAs of 256 threads per SM) that issues nothing but `iters` x 128 independent instructions per thread on ONE
+ * pipe: pipe 0 = scalar FP32 FMA (the FP32 non-tensor issue roofline), 1 = MUFU.EX2 (the special-function pipe that
+ * binds the FP32 sech^2 kernel), 2 = FP64 FMA.  *lane_ops (nullable) receives the number of thread-level instructions
+ * the launch executes and *n_sms (nullable) the SM count, so that the caller, timing the launch with its own events,
+ * gets lanes per clock and SM = lane_ops / (seconds x SM clock x n_sms).  d_sink: >= 4 bytes of device memory, not
+ * written in practice.  1 <= iters <= 2^32; else, or for an unknown pipe or a NULL d_sink, WL_ERR_INVALID_ARG. */
+wl_status wl_pipe_probe(int pipe, int64_t iters, float* d_sink, void* stream, int64_t* lane_ops, int* n_sms);
+
 /* Number of kernels wl_eval enqueues for these sizes (for launch accounting). */
 int wl_eval_launch_count(int64_t n_loops, int n_ppl, int n_T, int n_rho, int n_groups,
                          wl_dtype compute);

@@ -104,6 +104,8 @@ _lib.wl_eval_host.argtypes = [_vp, _vp, _int, _i64, _int, _dp, _int, _dp, _dp, _
                               _dp]
 _lib.wl_eval_host_trim.restype = _int
 _lib.wl_eval_host_trim.argtypes = []
+_lib.wl_pipe_probe.restype = _int
+_lib.wl_pipe_probe.argtypes = [_int, _i64, _vp, _vp, C.POINTER(C.c_int64), C.POINTER(C.c_int)]
 _lib.wl_status_string.restype = C.c_char_p
 _lib.wl_status_string.argtypes = [_int]
 _lib.wl_version.restype = C.c_char_p
@@ -486,6 +488,15 @@ def wl_eval_host(field, loops, T, rho_cm, phi_cm=None, n_groups=2, compute=torch
 def wl_eval_host_trim():
     """Returns the unused memory of wl_eval_host's private pool to the device."""
     _check(_lib.wl_eval_host_trim(), "wl_eval_host_trim")
+
+
+def wl_pipe_probe(pipe, iters, sink, stream=None):
+    """Enqueues the single-pipe instruction stream `pipe` (0 FFMA, 1 MUFU.EX2, 2 DFMA); returns (lane_ops, n_sms)."""
+    ops, sms = C.c_int64(0), C.c_int(0)
+    with torch.cuda.device(sink.device):
+        _check(_lib.wl_pipe_probe(int(pipe), int(iters), _ptr(sink), _stream(stream), C.byref(ops), C.byref(sms)),
+               "wl_pipe_probe")
+    return int(ops.value), int(sms.value)
 
 
 def wl_proper_time_nodes(a, Tmax, n_T) -> np.ndarray:

@@ -15,7 +15,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 LIB = os.path.join(HERE, "libwl.so")
-SOURCES = ("wl_api.cu", "wl_host.cu", "wl_eval_kernels.cu", "wl_wilson_sech2_f32.cu", "wl_wilson_sech2_f64.cu", "wl_wilson_fluxtube_f32.cu", "wl_generate_finalize.cu", "wl_action.cu", "wl_eval_static.cu")
+SOURCES = ("wl_api.cu", "wl_host.cu", "wl_eval_kernels.cu", "wl_wilson_sech2_f32.cu", "wl_wilson_sech2_f64.cu", "wl_wilson_fluxtube_f32.cu", "wl_generate_finalize.cu", "wl_action.cu", "wl_eval_static.cu", "wl_pipe_probe.cu")
 HEADERS = ("wl_internal.cuh", "wl_field_device.cuh", "wl_dloop_device.cuh", "wl_wilson_body.cuh", "wl_terms_generic.cuh",
            "wl_terms_packed_f32.cuh", "wl_terms_sech2_f64.cuh", "wl_block_bounds.cuh")
 

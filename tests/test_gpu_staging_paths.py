@@ -9,7 +9,9 @@ kernels that the bulk variant is compiled for) and small enough for compute-sani
 
     compute-sanitizer --tool memcheck|racecheck|synccheck python -m pytest tests/test_gpu_staging_paths.py -q
 
-(profiles/r03_sanitizer.md holds the output).  As an ordinary test it checks what must hold between the paths:
+(profiles/r03_sanitizer.md: the tool is closed on this GPU pool, so what stands in is this test's own evidence: every
+path repeated with bit-identical results, and three differently staged paths agreeing bit for bit).  It checks what
+must hold between the paths:
 same bits for default / bulk / seeded staging, level N of the discretisation estimate equal to the plain
 evaluation, shuffled groups summing to the same total.
 """
@@ -50,6 +52,14 @@ def test_all_staging_paths_agree(profile, params, compute):
     torch.cuda.synchronize()
 
     assert torch.isfinite(g0).all()
+    # a race in any of the three places would show as bits that change from run to run: every path three more times
+    for _ in range(3):
+        ra = api.wl_eval(f, loops, T, rho, None, n_groups=G, compute=compute)[1]
+        rb = api.wl_eval(f, loops, T, rho, None, n_groups=G, compute=compute, options=api.wl_eval_options(staging=1))[1]
+        rc = api.wl_eval_seeded(f, SEED, N_LOOPS, N_PPL, T, rho, None, n_groups=G, compute=compute, storage=sdt)[1]
+        rd = api.wl_eval_discretization(f, loops, T, rho, None, n_groups=G, compute=compute)
+        torch.cuda.synchronize()
+        assert torch.equal(ra, g0) and torch.equal(rb, g0) and torch.equal(rc, g0) and torch.equal(rd, gs3)
     assert torch.equal(g0, g1) and torch.equal(m0, m1)            # same staged values, same walk order: same bits
     assert torch.equal(g0, g2) and torch.equal(m0, m2)
     # the three levels of eq. (48)-(50) are sums over stride-2 / stride-4 sub-worldlines, not the plain N-point sum:
